@@ -1,0 +1,185 @@
+"""Pins for the oracle's full deposit, census and patch path (oracle/psd_oracle.c O1-O6).
+
+Invariants fixed by the method itself: PAPER.md:39-45 (equal mass per Lagrangian cell, 6 tets
+tile it), Eq. 1 (density = sum of m/V over covering tets), PAPER.md:72 (patches).
+"""
+import numpy as np
+import pytest
+
+import psd_inputs
+
+
+def crossing_field(N, rms, seed=7, dtype="float64", stride=3):
+    return psd_inputs.zeldovich_positions(N, 24, 3, rms, seed, dtype=dtype, stride=stride)
+
+
+@pytest.mark.parametrize("N,G", [(4, 8), (4, 4), (6, 9), (5, 8), (8, 4)])
+@pytest.mark.parametrize("shift", [(0, 0, 0), (0.013, 0.4, 0.77)])
+def test_unperturbed_lattice_is_uniform(oracle, N, G, shift):
+    """An unperturbed (rigidly shifted) lattice deposits exactly M/G^3 everywhere -- also with
+    every vertex on a cell face (G = 2N, zero shift; Q7) and for non-power-of-two G (Q12)."""
+    pos = psd_inputs.lattice(N, shift=shift)
+    grid, st = oracle.deposit_uniform(pos, 1.0, 2.5, G)
+    assert st["n_tets"] == 6 * N ** 3 and st["n_inverted"] == 0 and st["n_degenerate"] == 0
+    assert np.allclose(grid, 2.5 / G ** 3, rtol=1e-12, atol=0)
+
+
+def test_sheared_torus_is_uniform(oracle):
+    """Q3: integer torus shear x -> x + y (mod 1) keeps the density exactly uniform and
+    exercises the minimum-image unwrap on every cell of the wrap plane."""
+    pos = psd_inputs.lattice(6, shift=(0.21, 0.05, 0.6), shear_xy=1)
+    grid, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 12)
+    assert np.allclose(grid, 1.0 / 12 ** 3, rtol=1e-12, atol=0)
+
+
+def test_box_length_and_units(oracle):
+    """L != 1: positions in [0,L); the mass per cell does not depend on the unit of length."""
+    pos = psd_inputs.lattice(4, L=3.0, shift=(0.3, 0.1, 0.2))
+    grid, _ = oracle.deposit_uniform(pos, 3.0, 1.0, 8)
+    assert np.allclose(grid, 1.0 / 512, rtol=1e-12)
+    p1 = crossing_field(6, 0.8)
+    g1, _ = oracle.deposit_uniform(p1, 1.0, 1.0, 12)
+    g3, _ = oracle.deposit_uniform(p1 * 4.0, 4.0, 1.0, 12)
+    assert np.allclose(g1, g3, rtol=1e-10, atol=1e-16)
+
+
+def test_mass_conservation_and_signed_cover(oracle):
+    """Pin 3 (sum grid = M) and pin 6 (signed-volume mode: every cell gets exactly one cell
+    volume for ANY displacement field -- degree-1 map of the torus), with inverted tets."""
+    pos = crossing_field(12, 2.0)   # every cell edge stays < L/2, so the unwrap is valid (Q4)
+    grid, st = oracle.deposit_uniform(pos, 1.0, 1.0, 24)
+    assert st["n_inverted"] > 0.3 * st["n_tets"]
+    assert abs(grid.sum() - 1.0) < 1e-12
+    assert (grid > 0).all()
+    signed, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 24, mode=oracle.MODE_SIGNED)
+    assert np.allclose(signed, 1.0, rtol=0, atol=1e-11)
+
+
+def test_fp32_positions_are_read_exactly(oracle):
+    """fp32 input == the same numbers handed over as fp64 (conversion is exact)."""
+    p32 = crossing_field(6, 1.0, dtype="float32", stride=4)
+    p64 = p32[..., :3].astype(np.float64).copy()
+    a, _ = oracle.deposit_uniform(p32, 1.0, 1.0, 12)
+    b, _ = oracle.deposit_uniform(p64, 1.0, 1.0, 12)
+    assert np.array_equal(a, b)
+
+
+def test_window_and_range_are_consistent_with_full(oracle):
+    pos = crossing_field(6, 1.5)
+    G = 12
+    full, st = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    win = oracle.deposit_window(pos, 1.0, 1.0, G, [10, 3, 0], [4, 5, 12])  # wraps in x
+    want = np.take(full, np.arange(10, 14) % G, axis=0)[:, 3:8, :]
+    assert np.allclose(win, want, rtol=1e-12, atol=1e-18)
+    acc = np.zeros((G, G, G))
+    n3 = 6 ** 3
+    for a, b in [(0, 50), (50, 51), (51, n3)]:
+        acc, _ = oracle.deposit_uniform_range(pos, 1.0, 1.0, G, a, b, grid=acc)
+    assert np.allclose(acc, full, rtol=1e-12, atol=1e-18)
+
+
+def test_all_particles_coincident_is_degenerate(oracle):
+    """Q6: V = 0 exactly -> the whole tet mass goes to the cell holding the centroid."""
+    pos = np.full((3, 3, 3, 3), 0.3)
+    grid, st = oracle.deposit_uniform(pos, 1.0, 1.0, 4)
+    assert st["n_degenerate"] == st["n_tets"] == 162
+    assert grid[1, 1, 1] == pytest.approx(1.0) and np.count_nonzero(grid) == 1
+
+
+def test_census_properties(oracle):
+    """O5: totals tie the census to the deposit's own candidate count (two code paths), to the
+    tile grid and to a brute-force count over cells on a tiny input."""
+    pos = crossing_field(8, 2.0)
+    G = 16
+    c = oracle.census(pos, 1.0, G)
+    _, st = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    assert c["n_tets"] == 6 * 8 ** 3 == int(c["hist_tet"].sum())
+    assert c["sum_cells"] == st["n_candidates"]
+    assert c["n_inverted"] == st["n_inverted"]
+    assert c["n_pairs"] == int(c["tile_counts"].sum()) == int(c["hist_pair"].sum())
+    assert c["max_cells"] <= 2 ** (np.nonzero(c["hist_tet"])[0].max())
+    # brute force with the single-tet entry point
+    nt = G // 8
+    tc = np.zeros((nt, nt, nt), dtype=np.int64)
+    for i in range(8):
+        for j in range(8):
+            for k in range(8):
+                for t in range(6):
+                    _, _, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+                    tiles = [sorted({(x % G) // 8 for x in range(lo[a], hi[a] + 1)}) for a in range(3)]
+                    for a in tiles[0]:
+                        for b in tiles[1]:
+                            for d in tiles[2]:
+                                tc[a, b, d] += 1
+    assert np.array_equal(tc.ravel(), c["tile_counts"].astype(np.int64))
+
+
+def test_patches_level0_equals_uniform_and_restriction(oracle):
+    """Q13: level-0 patches tiled together = deposit_uniform(base_G); every coarse cell equals
+    the sum of its 8 children where refined."""
+    pos = crossing_field(8, 1.5, dtype="float32", stride=4)
+    base_G, P = 8, 4
+    patches = [[0, a, b, c] for a in range(2) for b in range(2) for c in range(2)]
+    patches += [[1, a, b, c] for a in (2, 3) for b in (0, 1) for c in (3, 0)]   # children of (1,0,1),(1,0,0)
+    patches += [[2, 7, 1, 0], [2, 0, 0, 7]]
+    patches = np.array(patches, dtype=np.int32)
+    mass = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches)
+    uni0, _ = oracle.deposit_uniform(pos, 1.0, 1.0, base_G)
+    uni1, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 2 * base_G)
+    uni2, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 4 * base_G)
+    for q, (l, a, b, c) in enumerate(patches):
+        ref = (uni0, uni1, uni2)[l][a * P:(a + 1) * P, b * P:(b + 1) * P, c * P:(c + 1) * P]
+        assert np.allclose(mass[q], ref, rtol=1e-11, atol=1e-18)
+    coarse = uni0.reshape(base_G, 1, base_G, 1, base_G, 1)
+    fine = uni1.reshape(base_G, 2, base_G, 2, base_G, 2).sum(axis=(1, 3, 5))
+    assert np.allclose(fine, coarse[:, 0, :, 0, :, 0], rtol=1e-11)
+
+
+def test_patch_counts_and_refine_rule(oracle):
+    """PAPER.md:66 refinement by tet count; Q14 rules on integer counts."""
+    pos = crossing_field(16, 2.5, dtype="float32", stride=4)
+    base_G, P = 32, 4
+    counts = [oracle.patch_counts(pos, 1.0, base_G, P, l) for l in range(3)]
+    c0 = oracle.census(pos, 1.0, base_G, tile=P)
+    assert np.array_equal(counts[0].ravel(), c0["tile_counts"].astype(np.uint64))
+    pl = oracle.refine_patches(counts, 2.0)
+    lv = pl[:, 0]
+    assert (lv == 0).sum() == 8 ** 3
+    assert (lv == 1).sum() % 8 == 0 and (lv == 2).sum() % 8 == 0
+    assert (lv == 1).sum() > 0
+    have = {tuple(r) for r in pl.tolist()}
+    for l, a, b, c in pl.tolist():          # every patch's parent exists
+        if l:
+            assert (l - 1, a // 2, b // 2, c // 2) in have
+    hot2 = np.argwhere(counts[2] > 2.0 * counts[2].astype(float).mean())
+    for a, b, c in hot2.tolist():           # every hot level-2 candidate is present
+        assert (2, a, b, c) in have
+    lit = oracle.refine_patches(counts, 1.2, rule=oracle.RULE_LITERAL_TOP_DOWN)
+    assert (lit[:, 0] == 0).sum() == 8 ** 3
+
+
+def test_input_generator_is_seeded_and_matches_recipe():
+    a = psd_inputs.config_positions(0)
+    b = psd_inputs.config_positions(0)
+    assert a.dtype == np.float64 and a.shape == (32, 32, 32, 3)
+    assert psd_inputs.sha256_of(a) == psd_inputs.sha256_of(b)
+    q = np.arange(32) / 32.0
+    d = a.copy()
+    d[..., 0] -= q[:, None, None]; d[..., 1] -= q[None, :, None]; d[..., 2] -= q[None, None, :]
+    d = (d + 0.5) % 1.0 - 0.5
+    assert np.isclose(np.sqrt(np.mean(d * d)) * 32, 0.3, rtol=1e-9)
+    from psd_inputs import zeldovich as z
+    k, g, phi = z._draw_modes(5, 40, 4)
+    assert len({tuple(x) for x in k.tolist()}) == 40 and ((k * k).sum(1) <= 16).all()
+    assert np.abs(z.displacement_direct(16, k, g, phi) - z.displacement_fft(16, k, g, phi)).max() < 1e-12
+    # curl-free: displacement parallel to k for a single mode
+    p1 = z.displacement_direct(8, k[:1], g[:1], phi[:1])
+    assert np.abs(np.cross(p1.reshape(-1, 3), k[0].astype(float))).max() < 1e-12
+
+
+def test_cfg0_has_no_shell_crossing(oracle):
+    """BASELINE.json configs[0]: 'no shell crossing' -> no inverted tets; mass conserved."""
+    pos = psd_inputs.config_positions(0)
+    grid, st = oracle.deposit_uniform(pos, 1.0, 1.0, 64)
+    assert st["n_tets"] == 196608 and st["n_inverted"] == 0
+    assert abs(grid.sum() - 1.0) < 1e-12
