@@ -1,0 +1,168 @@
+/*
+ * psd.h -- C ABI of libpsd: B200 (sm_100a) phase-space-element mass deposit.
+ *
+ * The operation (R. Kaehler, arXiv:1612.09491; citations are PAPER.md:LINE of the paper
+ * text): N^3 tracer particles stored in Lagrangian order define N^3 periodic Lagrangian
+ * cells; each cell is split into 6 tetrahedra of equal mass
+ * m = M/(6 N^3); every tetrahedron T is intersected exactly with every
+ * cubical deposit cell C it overlaps and
+ *
+ *        mass[C] += m * vol(T n C) / |vol(T)|            (PAPER.md:45-48 Eq. 1, :137)
+ *
+ * on a uniform periodic grid or on a list of cubical patches of an oct-tree.
+ *
+ * Conventions
+ *  - All pointers named *_dev are DEVICE pointers on the context's device, *_host are HOST
+ *    pointers.  No torch / C++ types cross this boundary.
+ *  - The caller owns positions and outputs; the context owns its scratch (pair lists,
+ *    counters), grown on demand and reused between calls.
+ *  - Every function returns a psd_status (0 = PSD_OK); nothing throws or exits.
+ *    psd_last_error() gives a human-readable string for the last failure on that context.
+ *  - Work is enqueued on the context's CUDA stream and is asynchronous unless stated;
+ *    psd_sync / psd_get_stats / psd_refine_patches / *_host calls synchronise.
+ *  - One context is used from one host thread at a time.
+ *  - There is no CPU fallback: without a CUDA device psd_create fails.
+ */
+#ifndef PSD_H
+#define PSD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psd_ctx psd_ctx;
+
+typedef enum {
+    PSD_OK = 0,
+    PSD_ERR_INVALID_ARG = 1, /* bad size / pointer / option                         */
+    PSD_ERR_STATE = 2,       /* deposit or refine before psd_build_tets             */
+    PSD_ERR_OOM = 3,         /* scratch allocation failed                           */
+    PSD_ERR_CUDA = 4,        /* a CUDA call or kernel failed (see psd_last_error)   */
+    PSD_ERR_UNWRAP = 5       /* reserved: minimum-image unwrap not valid            */
+} psd_status;
+
+enum { PSD_F32 = 0, PSD_F64 = 1 };
+
+/* psd_set_option keys */
+enum {
+    PSD_OPT_WEIGHT_MODE = 0, /* 0 (default): mass m/|V|.  1: signed volume, weight sign(det) in
+                                cell-volume units -- every cell then receives exactly 1.0 for
+                                any displacement field (a self-check needing no oracle).     */
+    PSD_OPT_KERNEL = 1,      /* 0 (default): binned tile path when the grid allows it (G % 8 == 0).
+                                1: direct path (one thread per tet, global atomics).           */
+    PSD_OPT_COUNTERS = 2,    /* 1: also count column tasks / face clips / plane clips / cells
+                                written during deposits (slower; for the roofline model).       */
+    PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 1024) */
+    PSD_OPT_CHORD_AXIS = 4   /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
+};
+
+/* refinement rules (reading Q14 of PAPER.md:66) */
+enum { PSD_RULE_LITERAL_TOP_DOWN = 0, PSD_RULE_BOTTOM_UP_LEVEL_MEAN = 1 };
+
+/* One cubical patch of the block-structured oct-tree: it covers the cells
+ * [o*P, o*P+P) per axis of the level grid with G_l = base_G * 2^level cells per side. */
+typedef struct {
+    int32_t level;
+    int32_t ox, oy, oz;
+} psd_patch;
+
+typedef struct {
+    int64_t n_tets;       /* 6 N^3                                                       */
+    int64_t n_tiles;      /* tiles (8^3 cells) of the last binned deposit                */
+    int64_t n_pairs;      /* (tet, tile) pairs = sum of tile_counts                      */
+    int64_t n_work_items; /* chunks of pair lists scheduled                              */
+    int64_t sum_cells;    /* sum over tets of AABB cells (candidate cells)               */
+    int64_t max_cells;    /* largest AABB                                                */
+    int64_t n_inverted;   /* tets with negative determinant                */
+    int64_t n_degenerate; /* tets with determinant exactly 0                             */
+    int64_t n_unwrap_suspect; /* unwrapped Lagrangian cell edges longer than L/4         */
+    int64_t n_nonfinite;  /* NaN/Inf position components seen by psd_build_tets          */
+    uint64_t hist_tet[64];  /* tets by b = bit_width(n_cells-1)                          */
+    uint64_t hist_pair[64]; /* pairs by b of the tet's cells inside that tile            */
+    /* PSD_OPT_COUNTERS = 1 only: */
+    int64_t n_column_tasks; /* (tet, column) tasks run                                   */
+    int64_t n_face_clips;   /* tet faces clipped to a column with non-empty result       */
+    int64_t n_plane_clips;  /* chord-plane clips of a face polygon                       */
+    int64_t n_cells_written;/* cell contributions added to accumulators                  */
+    /* device pointer to the per-tile counts of the last binned deposit (n_tiles uint32) */
+    const uint32_t* tile_counts_dev;
+    /* device time of the phases of the last deposit, ms (0 if not recorded)             */
+    float ms_census, ms_scan, ms_scatter, ms_deposit, ms_total;
+} psd_stats;
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the
+ * legacy default stream) that all work of this context is enqueued on; it must outlive
+ * the context. */
+int psd_create(psd_ctx** out, int device, void* cuda_stream);
+
+/* Frees only context-owned scratch.  NULL is allowed. */
+void psd_destroy(psd_ctx* ctx);
+
+/* PAPER.md:39-45, :60.  Register the particle set the tets are generated from.
+ *   pos_dev      N^3 particles in Lagrangian order: particle (i,j,k) at element offset
+ *                ((i*N+j)*N+k)*stride_elems, components x,y,z first (a 4th is ignored).
+ *                BORROWED: must stay valid and unchanged until the last deposit using it.
+ *   dtype        PSD_F32 or PSD_F64;  stride_elems 3 or 4 (4 with PSD_F32 = float4 loads).
+ *   N            particles per side, >= 2 (6 N^3 must fit uint32: N <= 894).
+ *   L            periodic box length > 0; positions are in [0, L] per axis.
+ *   total_mass   M; every tet carries m = M/(6 N^3).
+ * Tets are implicit (generated on the fly with minimum-image unwrapping relative to the
+ * cell's corner 0; valid while every cell edge is shorter than L/2): nothing is stored.
+ * Runs one validation pass over the positions and synchronises; non-finite positions give
+ * PSD_ERR_INVALID_ARG. */
+int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elems, int N, double L,
+                   double total_mass);
+
+/* PAPER.md:137, :155-161.  Deposit all 6 N^3 tets onto the uniform periodic grid.
+ *   G          cells per side (>= 1); cell (ix,iy,iz) spans [ix,ix+1)*L/G ...
+ *   grid_dev   G^3 doubles, index (ix*G+iy)*G+iz, MASS per cell (not density).
+ *   accumulate 0: the library zeroes the grid first; 1: adds to what is there.
+ * Asynchronous. */
+int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate);
+
+/* PAPER.md:66 (refinement by tet count), :72 (leaf patches).  Census-driven construction of
+ * the patch list: counts, per level l = 0..max_level, the tets whose cell range meets each
+ * candidate patch position of the level grid, then applies `rule` with `factor` on the host.
+ *   base_G, P    level-0 grid and cells per patch side (base_G % P == 0)
+ *   out_host     receives the patches ordered by level then (ox,oy,oz); cap = its capacity
+ *   n_out        number of patches (also when cap is too small: then PSD_ERR_INVALID_ARG)
+ *   counts_host  optional: receives the dense count arrays of all levels, concatenated
+ *                (sum over l of (base_G/P * 2^l)^3 uint64)
+ * Synchronous. */
+int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
+                       psd_patch* out_host, int64_t cap, int64_t* n_out, uint64_t* counts_host);
+
+/* PAPER.md:72, Q13.  Deposit into every listed patch the full contribution of
+ * every tet that overlaps it, on the patch's own level grid.
+ *   patches_host  n_patch patches (host; copied), distinct
+ *   P             cells per patch side, multiple of 8;  base_G % P == 0
+ *   mass_dev      n_patch * P^3 doubles, patch-major then (x*P+y)*P+z
+ * Asynchronous (the patch list is copied before return). */
+int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_patch, int P,
+                        int base_G, double* mass_dev, int accumulate);
+
+/* End-to-end convenience used for the host-buffer measurement: copies positions host->device,
+ * registers them, deposits, copies the G^3 grid device->host.  Synchronous.  Host buffers
+ * should be pinned for full copy bandwidth. */
+int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
+                             double L, double total_mass, int G, double* grid_host);
+
+/* Synchronises, then fills *out with the counters of the last build / deposit. */
+int psd_get_stats(psd_ctx* ctx, psd_stats* out);
+
+int psd_set_option(psd_ctx* ctx, int key, double value);
+int psd_sync(psd_ctx* ctx);
+const char* psd_last_error(const psd_ctx* ctx);
+
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
+int64_t psd_launch_count(const psd_ctx* ctx);
+
+/* Library identification: "libpsd sm_100a <build date>" */
+const char* psd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSD_H */

@@ -1,0 +1,538 @@
+// psd_abi.cu -- host side of libpsd: context, scratch management, launch order, C ABI.
+// See include/psd.h for the contract of every entry point.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/psd.h"
+#include "psd_kernels.cuh"
+
+using namespace psd;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        size_t want = bytes + bytes / 8 + 256;  // a little slack so small growth does not realloc
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { e = cudaMalloc(&p, bytes); want = bytes; }
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+}  // namespace
+
+struct psd_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    Particles part{};
+    bool built = false;
+    double total_mass = 0.0;
+    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = 0;
+    unsigned int chunk = 1024;
+    DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
+        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid;
+    unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
+    psd_stats last{};
+    bool stats_pending = false;
+    bool binned_last = false;
+    std::string err;
+    int64_t launches = 0;
+    cudaEvent_t ev[6] = {};
+};
+
+namespace {
+
+int fail(psd_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+int cuda_fail(psd_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, e == cudaErrorMemoryAllocation ? PSD_ERR_OOM : PSD_ERR_CUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                    \
+    do {                                                            \
+        cudaError_t _e = (call);                                    \
+        if (_e != cudaSuccess) return cuda_fail(ctx, _e, #call);    \
+    } while (0)
+
+constexpr int PINNED_WORDS = ST_COUNT + 128 + 2;
+
+int reset_stats(psd_ctx* ctx) {
+    CK(ctx->stats.ensure(sizeof(unsigned long long) * ST_COUNT));
+    CK(ctx->hist.ensure(sizeof(unsigned long long) * 128));
+    CK(cudaMemsetAsync(ctx->stats.p, 0, sizeof(unsigned long long) * ST_COUNT, ctx->stream));
+    CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(unsigned long long) * 128, ctx->stream));
+    return PSD_OK;
+}
+
+// census + scan + scatter + items + tile deposit over `n_tiles` tiles of `space`
+int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
+    cudaStream_t st = ctx->stream;
+    const long long ncell = (long long)ctx->part.N * ctx->part.N * ctx->part.N;
+    CK(ctx->tile_counts.ensure(sizeof(unsigned int) * n_tiles));
+    CK(ctx->cursors.ensure(sizeof(unsigned int) * n_tiles));
+    CK(ctx->tile_offsets.ensure(sizeof(unsigned long long) * (n_tiles + 1)));
+    CK(ctx->item_offsets.ensure(sizeof(unsigned long long) * (n_tiles + 1)));
+    const int nparts = (int)((n_tiles + SCAN_BLOCK - 1) / SCAN_BLOCK);
+    CK(ctx->part_pairs.ensure(sizeof(unsigned long long) * nparts));
+    CK(ctx->part_items.ensure(sizeof(unsigned long long) * nparts));
+    CK(ctx->totals.ensure(sizeof(unsigned long long) * 2));
+    CK(cudaMemsetAsync(ctx->tile_counts.p, 0, sizeof(unsigned int) * n_tiles, st));
+    CK(cudaMemsetAsync(ctx->cursors.p, 0, sizeof(unsigned int) * n_tiles, st));
+    int rc = reset_stats(ctx);
+    if (rc) return rc;
+
+    CK(cudaEventRecord(ctx->ev[0], st));
+    const int cb = 256;
+    const unsigned int cgrid = (unsigned int)((ncell + cb - 1) / cb);
+    k_census<false><<<cgrid, cb, 0, st>>>(ctx->part, space, ctx->tile_counts.as<unsigned int>(), nullptr,
+                                          nullptr, nullptr, ctx->stats.as<unsigned long long>(),
+                                          ctx->hist.as<unsigned long long>());
+    CK(cudaEventRecord(ctx->ev[1], st));
+    k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk,
+                                                   ctx->part_pairs.as<unsigned long long>(),
+                                                   ctx->part_items.as<unsigned long long>());
+    k_scan_top<<<1, SCAN_BLOCK, 0, st>>>(ctx->part_pairs.as<unsigned long long>(),
+                                         ctx->part_items.as<unsigned long long>(), nparts,
+                                         ctx->totals.as<unsigned long long>());
+    k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk,
+                                                ctx->part_pairs.as<unsigned long long>(),
+                                                ctx->part_items.as<unsigned long long>(),
+                                                ctx->tile_offsets.as<unsigned long long>(),
+                                                ctx->item_offsets.as<unsigned long long>());
+    ctx->launches += 4;
+    CK(cudaGetLastError());
+    // the only host round trip of a deposit: list sizes, to size the scratch and the grid
+    CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 128, ctx->totals.p, sizeof(unsigned long long) * 2,
+                       cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const unsigned long long n_pairs = ctx->pinned[ST_COUNT + 128], n_items = ctx->pinned[ST_COUNT + 129];
+    ctx->last.n_pairs = (int64_t)n_pairs;
+    ctx->last.n_work_items = (int64_t)n_items;
+    ctx->last.n_tiles = n_tiles;
+    CK(cudaEventRecord(ctx->ev[2], st));
+    if (n_pairs > 0) {
+        if (n_items > 0x7fffffffull) return fail(ctx, PSD_ERR_INVALID_ARG, "too many work items");
+        CK(ctx->pair_ids.ensure(sizeof(unsigned int) * n_pairs));
+        CK(ctx->items.ensure(sizeof(Item) * n_items));
+        k_items<<<(unsigned int)((n_tiles + 255) / 256), 256, 0, st>>>(
+            ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
+            ctx->item_offsets.as<unsigned long long>(), ctx->items.as<Item>());
+        k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
+                                             ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
+                                             nullptr, nullptr);
+        ctx->launches += 2;
+        CK(cudaEventRecord(ctx->ev[3], st));
+        DepositArgs A;
+        A.part = ctx->part;
+        A.space = space;
+        A.pair_ids = ctx->pair_ids.as<unsigned int>();
+        A.items = ctx->items.as<Item>();
+        A.mass_per_tet = ctx->total_mass / (6.0 * (double)ncell);
+        A.weight_mode = ctx->weight_mode;
+        A.chord_axis = ctx->chord_axis;
+        A.stats = ctx->stats.as<unsigned long long>();
+        if (ctx->counters)
+            k_deposit_tiles<true><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+        else
+            k_deposit_tiles<false><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+        ctx->launches += 1;
+    } else {
+        CK(cudaEventRecord(ctx->ev[3], st));
+    }
+    CK(cudaEventRecord(ctx->ev[4], st));
+    CK(cudaGetLastError());
+    ctx->stats_pending = true;
+    ctx->binned_last = true;
+    return PSD_OK;
+}
+
+int run_direct(psd_ctx* ctx, Space space) {
+    cudaStream_t st = ctx->stream;
+    const long long ncell = (long long)ctx->part.N * ctx->part.N * ctx->part.N;
+    const long long ntet = 6 * ncell;
+    int rc = reset_stats(ctx);
+    if (rc) return rc;
+    CK(cudaEventRecord(ctx->ev[0], st));
+    k_tet_stats<<<(unsigned int)((ntet + 255) / 256), 256, 0, st>>>(
+        ctx->part, (double)space.G / space.L, ctx->stats.as<unsigned long long>(), ctx->hist.as<unsigned long long>());
+    CK(cudaEventRecord(ctx->ev[1], st));
+    CK(cudaEventRecord(ctx->ev[2], st));
+    CK(cudaEventRecord(ctx->ev[3], st));
+    DepositArgs A;
+    A.part = ctx->part;
+    A.space = space;
+    A.pair_ids = nullptr;
+    A.items = nullptr;
+    A.mass_per_tet = ctx->total_mass / (6.0 * (double)ncell);
+    A.weight_mode = ctx->weight_mode;
+    A.chord_axis = ctx->chord_axis;
+    A.stats = ctx->stats.as<unsigned long long>();
+    const unsigned int grid = (unsigned int)((ntet + 127) / 128);
+    if (ctx->counters) k_deposit_direct<true><<<grid, 128, 0, st>>>(A);
+    else k_deposit_direct<false><<<grid, 128, 0, st>>>(A);
+    ctx->launches += 2;
+    CK(cudaEventRecord(ctx->ev[4], st));
+    CK(cudaGetLastError());
+    ctx->last.n_pairs = 0; ctx->last.n_work_items = 0; ctx->last.n_tiles = 0;
+    ctx->stats_pending = true;
+    ctx->binned_last = false;
+    return PSD_OK;
+}
+
+bool valid_ctx(psd_ctx* ctx) { return ctx != nullptr; }
+
+}  // namespace
+
+extern "C" {
+
+int psd_create(psd_ctx** out, int device, void* cuda_stream) {
+    if (!out) return PSD_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0 || device < 0 || device >= ndev) return PSD_ERR_CUDA;
+    psd_ctx* ctx = new (std::nothrow) psd_ctx();
+    if (!ctx) return PSD_ERR_OOM;
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->pinned, sizeof(unsigned long long) * PINNED_WORDS);
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreate(&ctx->ev[i]);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_tiles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
+    if (e != cudaSuccess) {
+        psd_destroy(ctx);
+        return PSD_ERR_CUDA;
+    }
+    *out = ctx;
+    return PSD_OK;
+}
+
+void psd_destroy(psd_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    DevBuf* bufs[] = {&ctx->tile_counts, &ctx->cursors, &ctx->tile_offsets, &ctx->item_offsets, &ctx->items,
+                      &ctx->pair_ids, &ctx->part_pairs, &ctx->part_items, &ctx->totals, &ctx->stats, &ctx->hist,
+                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid};
+    for (DevBuf* b : bufs) b->release();
+    if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    for (int i = 0; i < 6; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+}
+
+int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elems, int N, double L,
+                   double total_mass) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    ctx->built = false;
+    if (!pos_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "pos_dev is NULL");
+    if (dtype != PSD_F32 && dtype != PSD_F64) return fail(ctx, PSD_ERR_INVALID_ARG, "dtype must be PSD_F32 or PSD_F64");
+    if (stride_elems != 3 && stride_elems != 4) return fail(ctx, PSD_ERR_INVALID_ARG, "stride_elems must be 3 or 4");
+    if (N < 2 || N > 894) return fail(ctx, PSD_ERR_INVALID_ARG, "N must be in [2, 894]");
+    if (!(L > 0.0) || !std::isfinite(L)) return fail(ctx, PSD_ERR_INVALID_ARG, "L must be finite and > 0");
+    if (!std::isfinite(total_mass)) return fail(ctx, PSD_ERR_INVALID_ARG, "total_mass must be finite");
+    if (dtype == PSD_F32 && stride_elems == 4 && (reinterpret_cast<uintptr_t>(pos_dev) & 15))
+        return fail(ctx, PSD_ERR_INVALID_ARG, "float4 positions must be 16-byte aligned");
+    CK(cudaSetDevice(ctx->device));
+    ctx->part.pos = pos_dev;
+    ctx->part.dtype = dtype;
+    ctx->part.stride = stride_elems;
+    ctx->part.N = N;
+    ctx->part.L = L;
+    ctx->total_mass = total_mass;
+    int rc = reset_stats(ctx);
+    if (rc) return rc;
+    k_validate<<<1184, 256, 0, ctx->stream>>>(ctx->part, ctx->stats.as<unsigned long long>());
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(ctx->pinned, ctx->stats.p, sizeof(unsigned long long) * ST_COUNT, cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    std::memset(&ctx->last, 0, sizeof(ctx->last));
+    ctx->last.n_tets = 6ll * N * N * N;
+    ctx->last.n_nonfinite = (int64_t)ctx->pinned[ST_NONFINITE];
+    ctx->stats_pending = false;
+    if (ctx->last.n_nonfinite) return fail(ctx, PSD_ERR_INVALID_ARG, "positions contain NaN or Inf");
+    ctx->built = true;
+    return PSD_OK;
+}
+
+int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    if (!ctx->built) return fail(ctx, PSD_ERR_STATE, "psd_deposit_uniform before psd_build_tets");
+    if (G < 1 || G > 2048) return fail(ctx, PSD_ERR_INVALID_ARG, "G must be in [1, 2048]");
+    if (!grid_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "grid_dev is NULL");
+    CK(cudaSetDevice(ctx->device));
+    if (!accumulate) CK(cudaMemsetAsync(grid_dev, 0, sizeof(double) * (size_t)G * G * G, ctx->stream));
+    Space s{};
+    s.patch_mode = 0;
+    s.G = G;
+    s.nt = G / TILE;
+    s.out = grid_dev;
+    s.L = ctx->part.L;
+    const int64_t nf = ctx->last.n_nonfinite;
+    std::memset(&ctx->last, 0, sizeof(ctx->last));
+    ctx->last.n_tets = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
+    ctx->last.n_nonfinite = nf;
+    if (ctx->kernel == 1 || G % TILE != 0) return run_direct(ctx, s);
+    return run_binned(ctx, s, (long long)s.nt * s.nt * s.nt);
+}
+
+int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_patch, int P, int base_G,
+                        double* mass_dev, int accumulate) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    if (!ctx->built) return fail(ctx, PSD_ERR_STATE, "psd_deposit_patches before psd_build_tets");
+    if (!patches_host || n_patch < 1 || !mass_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "NULL argument or no patches");
+    if (P < TILE || P % TILE || base_G < P || base_G % P)
+        return fail(ctx, PSD_ERR_INVALID_ARG, "P must be a multiple of 8 and divide base_G");
+    CK(cudaSetDevice(ctx->device));
+    int max_level = 0;
+    for (int64_t q = 0; q < n_patch; ++q) {
+        const psd_patch& pp = patches_host[q];
+        if (pp.level < 0 || pp.level > 7) return fail(ctx, PSD_ERR_INVALID_ARG, "patch level out of range [0,7]");
+        long long np = ((long long)base_G << pp.level) / P;
+        if ((long long)base_G << pp.level > 2048 * 8)
+            return fail(ctx, PSD_ERR_INVALID_ARG, "level grid too fine");
+        if (pp.ox < 0 || pp.oy < 0 || pp.oz < 0 || pp.ox >= np || pp.oy >= np || pp.oz >= np)
+            return fail(ctx, PSD_ERR_INVALID_ARG, "patch origin outside its level grid");
+        if (pp.level > max_level) max_level = pp.level;
+    }
+    Space s{};
+    s.patch_mode = 1;
+    s.base_G = base_G;
+    s.P = P;
+    s.tp = P / TILE;
+    s.n_levels = max_level + 1;
+    s.L = ctx->part.L;
+    s.out = mass_dev;
+    long long total = 0;
+    for (int l = 0; l <= max_level; ++l) {
+        s.lookup_off[l] = total;
+        long long np = ((long long)base_G << l) / P;
+        total += np * np * np;
+    }
+    std::vector<int> lookup((size_t)total, -1);
+    for (int64_t q = 0; q < n_patch; ++q) {
+        const psd_patch& pp = patches_host[q];
+        long long np = ((long long)base_G << pp.level) / P;
+        long long idx = s.lookup_off[pp.level] + ((long long)pp.ox * np + pp.oy) * np + pp.oz;
+        if (lookup[(size_t)idx] != -1) return fail(ctx, PSD_ERR_INVALID_ARG, "duplicate patch in list");
+        lookup[(size_t)idx] = (int)q;
+    }
+    CK(ctx->lookup.ensure(sizeof(int) * (size_t)total));
+    CK(ctx->patches.ensure(sizeof(PatchDev) * (size_t)n_patch));
+    // pageable host memory: these copies complete before return, so the caller's list can go away
+    CK(cudaMemcpyAsync(ctx->lookup.p, lookup.data(), sizeof(int) * (size_t)total, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->patches.p, patches_host, sizeof(PatchDev) * (size_t)n_patch, cudaMemcpyHostToDevice,
+                       ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    s.lookup = ctx->lookup.as<int>();
+    s.patches = ctx->patches.as<PatchDev>();
+    if (!accumulate) CK(cudaMemsetAsync(mass_dev, 0, sizeof(double) * (size_t)n_patch * P * P * P, ctx->stream));
+    const int64_t nf = ctx->last.n_nonfinite;
+    std::memset(&ctx->last, 0, sizeof(ctx->last));
+    ctx->last.n_tets = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
+    ctx->last.n_nonfinite = nf;
+    return run_binned(ctx, s, (long long)n_patch * s.tp * s.tp * s.tp);
+}
+
+int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
+                       psd_patch* out_host, int64_t cap, int64_t* n_out, uint64_t* counts_host) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    if (!ctx->built) return fail(ctx, PSD_ERR_STATE, "psd_refine_patches before psd_build_tets");
+    if (!n_out || P < 1 || base_G < P || base_G % P || max_level < 0 || max_level > 7 || !(factor > 0.0) ||
+        (rule != PSD_RULE_LITERAL_TOP_DOWN && rule != PSD_RULE_BOTTOM_UP_LEVEL_MEAN))
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_refine_patches: bad argument");
+    if (((long long)base_G << max_level) > 2048 * 8) return fail(ctx, PSD_ERR_INVALID_ARG, "level grid too fine");
+    CK(cudaSetDevice(ctx->device));
+    const int nl = max_level + 1;
+    std::vector<long long> off(nl + 1, 0);
+    std::vector<int> np(nl);
+    for (int l = 0; l < nl; ++l) {
+        np[l] = (base_G << l) / P;
+        off[l + 1] = off[l] + (long long)np[l] * np[l] * np[l];
+    }
+    CK(ctx->refine_counts.ensure(sizeof(unsigned long long) * (size_t)off[nl]));
+    CK(cudaMemsetAsync(ctx->refine_counts.p, 0, sizeof(unsigned long long) * (size_t)off[nl], ctx->stream));
+    const long long ntet = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
+    for (int l = 0; l < nl; ++l) {
+        k_patch_counts<<<(unsigned int)((ntet + 255) / 256), 256, 0, ctx->stream>>>(
+            ctx->part, base_G, P, l, ctx->refine_counts.as<unsigned long long>() + off[l]);
+        ctx->launches += 1;
+    }
+    CK(cudaGetLastError());
+    std::vector<unsigned long long> cnt((size_t)off[nl]);
+    CK(cudaMemcpyAsync(cnt.data(), ctx->refine_counts.p, sizeof(unsigned long long) * cnt.size(),
+                       cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (counts_host) std::memcpy(counts_host, cnt.data(), sizeof(unsigned long long) * cnt.size());
+
+    // ---- the rule, on integers (Q14)
+    auto at = [&](int l, int a, int b, int c) -> size_t { return (size_t)(off[l] + ((long long)a * np[l] + b) * np[l] + c); };
+    std::vector<char> exists((size_t)off[nl], 0), split((size_t)off[nl], 0);
+    for (long long i = 0; i < off[1]; ++i) exists[(size_t)i] = 1;
+    if (rule == PSD_RULE_BOTTOM_UP_LEVEL_MEAN) {
+        // hot(l, pos): count > factor * mean of that level's counts, l >= 1
+        std::vector<char> hot((size_t)off[nl], 0);
+        for (int l = 1; l < nl; ++l) {
+            long double sum = 0;
+            for (long long i = off[l]; i < off[l + 1]; ++i) sum += (long double)cnt[(size_t)i];
+            double mean = (double)(sum / (long double)(off[l + 1] - off[l]));
+            for (long long i = off[l]; i < off[l + 1]; ++i) hot[(size_t)i] = (double)cnt[(size_t)i] > factor * mean;
+        }
+        for (int l = nl - 2; l >= 0; --l)
+            for (int a = 0; a < np[l]; ++a)
+                for (int b = 0; b < np[l]; ++b)
+                    for (int c = 0; c < np[l]; ++c) {
+                        char any = 0;
+                        for (int d = 0; d < 8; ++d) {
+                            size_t ch = at(l + 1, 2 * a + (d & 1), 2 * b + ((d >> 1) & 1), 2 * c + (d >> 2));
+                            any |= hot[ch] | split[ch];
+                        }
+                        split[at(l, a, b, c)] = any;
+                    }
+    } else {
+        long double sum = 0;
+        for (long long i = 0; i < off[1]; ++i) sum += (long double)cnt[(size_t)i];
+        double thr = factor * (double)(sum / (long double)off[1]);
+        for (int l = 0; l + 1 < nl; ++l)
+            for (long long i = off[l]; i < off[l + 1]; ++i) split[(size_t)i] = (double)cnt[(size_t)i] > thr;
+    }
+    for (int l = 0; l + 1 < nl; ++l)
+        for (int a = 0; a < np[l]; ++a)
+            for (int b = 0; b < np[l]; ++b)
+                for (int c = 0; c < np[l]; ++c) {
+                    size_t me = at(l, a, b, c);
+                    if (!(exists[me] && split[me])) continue;
+                    for (int d = 0; d < 8; ++d)
+                        exists[at(l + 1, 2 * a + (d & 1), 2 * b + ((d >> 1) & 1), 2 * c + (d >> 2))] = 1;
+                }
+    int64_t n = 0;
+    for (int l = 0; l < nl; ++l)
+        for (int a = 0; a < np[l]; ++a)
+            for (int b = 0; b < np[l]; ++b)
+                for (int c = 0; c < np[l]; ++c)
+                    if (exists[at(l, a, b, c)]) {
+                        if (out_host && n < cap) out_host[n] = psd_patch{l, a, b, c};
+                        ++n;
+                    }
+    *n_out = n;
+    if (out_host && n > cap) return fail(ctx, PSD_ERR_INVALID_ARG, "patch list capacity too small");
+    return PSD_OK;
+}
+
+int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N, double L,
+                             double total_mass, int G, double* grid_host) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    if (!pos_host || !grid_host) return fail(ctx, PSD_ERR_INVALID_ARG, "NULL host buffer");
+    if ((dtype != PSD_F32 && dtype != PSD_F64) || (stride_elems != 3 && stride_elems != 4) || N < 2 || N > 894 ||
+        G < 1 || G > 2048)
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_deposit_uniform_host: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    const size_t pbytes = (size_t)N * N * N * stride_elems * (dtype == PSD_F32 ? 4 : 8);
+    const size_t gbytes = sizeof(double) * (size_t)G * G * G;
+    CK(ctx->host_pos.ensure(pbytes));
+    CK(ctx->host_grid.ensure(gbytes));
+    CK(cudaMemcpyAsync(ctx->host_pos.p, pos_host, pbytes, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = psd_build_tets(ctx, ctx->host_pos.p, dtype, stride_elems, N, L, total_mass);
+    if (rc) return rc;
+    rc = psd_deposit_uniform(ctx, G, ctx->host_grid.as<double>(), 0);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(grid_host, ctx->host_grid.p, gbytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PSD_OK;
+}
+
+int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
+    if (!valid_ctx(ctx) || !out) return PSD_ERR_INVALID_ARG;
+    CK(cudaSetDevice(ctx->device));
+    if (ctx->stats_pending) {
+        CK(cudaMemcpyAsync(ctx->pinned, ctx->stats.p, sizeof(unsigned long long) * ST_COUNT, cudaMemcpyDeviceToHost,
+                           ctx->stream));
+        CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT, ctx->hist.p, sizeof(unsigned long long) * 128,
+                           cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        psd_stats& s = ctx->last;
+        s.sum_cells = (int64_t)ctx->pinned[ST_SUM_CELLS];
+        s.max_cells = (int64_t)ctx->pinned[ST_MAX_CELLS];
+        s.n_inverted = (int64_t)ctx->pinned[ST_INVERTED];
+        s.n_degenerate = (int64_t)ctx->pinned[ST_DEGENERATE];
+        s.n_unwrap_suspect = (int64_t)ctx->pinned[ST_UNWRAP];
+        s.n_column_tasks = (int64_t)ctx->pinned[ST_TASKS];
+        s.n_face_clips = (int64_t)ctx->pinned[ST_FACE_CLIPS];
+        s.n_plane_clips = (int64_t)ctx->pinned[ST_PLANE_CLIPS];
+        s.n_cells_written = (int64_t)ctx->pinned[ST_CELLS];
+        for (int i = 0; i < 64; ++i) {
+            s.hist_tet[i] = ctx->pinned[ST_COUNT + i];
+            s.hist_pair[i] = ctx->pinned[ST_COUNT + 64 + i];
+        }
+        s.tile_counts_dev = ctx->binned_last ? ctx->tile_counts.as<unsigned int>() : nullptr;
+        cudaEventElapsedTime(&s.ms_census, ctx->ev[0], ctx->ev[1]);
+        cudaEventElapsedTime(&s.ms_scan, ctx->ev[1], ctx->ev[2]);
+        cudaEventElapsedTime(&s.ms_scatter, ctx->ev[2], ctx->ev[3]);
+        cudaEventElapsedTime(&s.ms_deposit, ctx->ev[3], ctx->ev[4]);
+        cudaEventElapsedTime(&s.ms_total, ctx->ev[0], ctx->ev[4]);
+        ctx->stats_pending = false;
+    } else {
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    *out = ctx->last;
+    return PSD_OK;
+}
+
+int psd_set_option(psd_ctx* ctx, int key, double value) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    const int iv = (int)value;
+    switch (key) {
+        case PSD_OPT_WEIGHT_MODE:
+            if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "weight mode must be 0 or 1");
+            ctx->weight_mode = iv; return PSD_OK;
+        case PSD_OPT_KERNEL:
+            if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "kernel must be 0 or 1");
+            ctx->kernel = iv; return PSD_OK;
+        case PSD_OPT_COUNTERS:
+            ctx->counters = iv != 0; return PSD_OK;
+        case PSD_OPT_CHUNK:
+            if (iv < 32 || iv > (1 << 20)) return fail(ctx, PSD_ERR_INVALID_ARG, "chunk must be in [32, 2^20]");
+            ctx->chunk = (unsigned int)iv; return PSD_OK;
+        case PSD_OPT_CHORD_AXIS:
+            if (iv < -1 || iv > 2) return fail(ctx, PSD_ERR_INVALID_ARG, "chord axis must be -1..2");
+            ctx->chord_axis = iv; return PSD_OK;
+        default:
+            return fail(ctx, PSD_ERR_INVALID_ARG, "unknown option key");
+    }
+}
+
+int psd_sync(psd_ctx* ctx) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PSD_OK;
+}
+
+const char* psd_last_error(const psd_ctx* ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+
+int64_t psd_launch_count(const psd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* psd_version(void) { return "libpsd sm_100a " __DATE__; }
+
+}  // extern "C"

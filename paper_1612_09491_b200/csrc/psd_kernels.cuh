@@ -1,0 +1,603 @@
+// psd_kernels.cuh -- kernels of the deposit path (sm_100a).  Steps:
+//   a1 tet generation        load_tet_vertices / k_census / k_scatter / k_deposit_*
+//   a2 AABB + census         k_census      (per-tile counts, size-class histograms)
+//   a3 bin / sort            k_scan_* + k_scatter (counting sort of tet ids by tile) + k_items
+//   a4-a6 classify, clip, accumulate, flush    k_deposit_tiles (binned) / k_deposit_direct
+//   a7 patch path            the same kernels with Space::patch_mode = 1, k_patch_counts
+#pragma once
+#include "psd_geom.cuh"
+
+namespace psd {
+
+struct PatchDev { int level, ox, oy, oz; };
+
+// Where deposits go: a uniform periodic G^3 grid, or a list of P^3 patches on level grids.
+struct Space {
+    int patch_mode;
+    // uniform
+    int G;            // cells per side
+    int nt;           // tiles per side (G/8), binned path only
+    // patches
+    int base_G, P, tp;        // tp = P/8 tiles per patch side
+    int n_levels;
+    const PatchDev* patches;  // device
+    const int* lookup;        // dense patch-position -> patch index (or -1), levels concatenated
+    long long lookup_off[8];  // start of each level in lookup
+    double* out;
+    double L;
+};
+
+__device__ __forceinline__ double level_scale(const Space& s, int level) {
+    return s.patch_mode ? __ddiv_rn((double)(s.base_G << level), s.L) : __ddiv_rn((double)s.G, s.L);
+}
+__device__ __forceinline__ int level_G(const Space& s, int level) {
+    return s.patch_mode ? (s.base_G << level) : s.G;
+}
+
+struct Item { unsigned int tile; unsigned int count; unsigned long long begin; };
+
+enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
+       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_COUNT };
+
+// ---------------------------------------------------------------- validation of positions
+__global__ void k_validate(Particles p, unsigned long long* stats) {
+    int64_t n = (int64_t)p.N * p.N * p.N;
+    unsigned int bad = 0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        double v[3];
+        load_pos(p, i, v);
+        bad += !(isfinite(v[0]) && isfinite(v[1]) && isfinite(v[2]));
+    }
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&stats[ST_NONFINITE], (unsigned long long)bad);
+}
+
+// Enumerate the distinct periodic blocks (edge `bs` cells, `nb` per side) met by the cell range
+// [lo,hi] of one tet on a grid of Gl cells; f(bx,by,bz, cells_inside) once per block.
+template <class F>
+__device__ __forceinline__ void for_each_block(const int lo[3], const int hi[3], int Gl, int bs,
+                                               int nb, F f) {
+    int b0[3], cnt[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        b0[x] = floor_div(lo[x], bs);
+        cnt[x] = min(floor_div(hi[x], bs) - b0[x] + 1, nb);
+    }
+    for (int qx = 0; qx < cnt[0]; ++qx)
+        for (int qy = 0; qy < cnt[1]; ++qy)
+            for (int qz = 0; qz < cnt[2]; ++qz) {
+                int q[3] = {qx, qy, qz}, bw[3];
+                long long inside = 1;
+#pragma unroll
+                for (int x = 0; x < 3; ++x) {
+                    bw[x] = wrap_mod(b0[x] + q[x], nb);
+                    // cells of [lo,hi] whose wrapped position falls in block bw (all images)
+                    int first = bw[x] * bs;
+                    int m_lo = -floor_div(first + bs - 1 - lo[x], Gl);  // ceil((lo-first-bs+1)/Gl)
+                    int m_hi = floor_div(hi[x] - first, Gl);
+                    int c = 0;
+                    for (int m = m_lo; m <= m_hi; ++m) {
+                        int a = max(lo[x], first + m * Gl), b = min(hi[x], first + bs - 1 + m * Gl);
+                        c += max(b - a + 1, 0);
+                    }
+                    inside *= c;
+                }
+                f(bw[0], bw[1], bw[2], inside);
+            }
+}
+
+// tile id of wrapped tile coords on `level`; -1 if no patch there (patch mode)
+__device__ __forceinline__ long long tile_id_of(const Space& s, int level, int tx, int ty, int tz) {
+    if (!s.patch_mode) return ((long long)tx * s.nt + ty) * s.nt + tz;
+    int np = (s.base_G << level) / s.P;
+    int px = tx / s.tp, py = ty / s.tp, pz = tz / s.tp;
+    int pi = s.lookup[s.lookup_off[level] + ((long long)px * np + py) * np + pz];
+    if (pi < 0) return -1;
+    int sub = ((tx % s.tp) * s.tp + (ty % s.tp)) * s.tp + (tz % s.tp);
+    return (long long)pi * (s.tp * s.tp * s.tp) + sub;
+}
+
+// ---------------------------------------------------------------- a2 census / a3 scatter
+// One thread per Lagrangian cell (6 tets).  SCATTER = false: count pairs per tile + statistics.
+// SCATTER = true: write tet ids into the per-tile lists (counting sort, order within a tile is
+// the arrival order of the atomics).
+template <bool SCATTER>
+__global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned int* tile_counts,
+                                                const unsigned long long* tile_offsets,
+                                                unsigned int* cursors, unsigned int* pair_ids,
+                                                unsigned long long* stats,
+                                                unsigned long long* hist /* [2][64] */) {
+    __shared__ unsigned int sh_hist[2][64];
+    __shared__ unsigned long long sh_stat[ST_COUNT];
+    if (!SCATTER) {
+        for (int i = threadIdx.x; i < 128; i += blockDim.x) (&sh_hist[0][0])[i] = 0;
+        if (threadIdx.x < ST_COUNT) sh_stat[threadIdx.x] = 0;
+        __syncthreads();
+    }
+    const int N = p.N;
+    const int64_t ncell = (int64_t)N * N * N;
+    int64_t cell = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (cell < ncell) {
+        int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((int64_t)N * N));
+        double C[8][3];
+#pragma unroll
+        for (int b = 0; b < 8; ++b) load_pos(p, corner_index(i, j, k, b, N), C[b]);
+        unsigned int suspect = 0;
+#pragma unroll
+        for (int b = 1; b < 8; ++b)
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                C[b][x] = unwrap1(C[b][x], C[0][x], p.L);
+                if (!SCATTER && (b == 1 || b == 2 || b == 4))
+                    suspect |= fabs(C[b][x] - C[0][x]) > 0.25 * p.L;
+            }
+        if (!SCATTER && suspect) atomicAdd(&sh_stat[ST_UNWRAP], 1ull);
+        const int nlev = s.patch_mode ? s.n_levels : 1;
+        for (int level = 0; level < nlev; ++level) {
+            const double scale = level_scale(s, level);
+            const int Gl = level_G(s, level);
+            const int nb = Gl / TILE;
+#pragma unroll 1
+            for (int t6 = 0; t6 < 6; ++t6) {
+                double P[4][3];
+                int ca = c_kuhn_mid[t6][0], cb = c_kuhn_mid[t6][1];
+#pragma unroll
+                for (int x = 0; x < 3; ++x) {
+                    P[0][x] = C[0][x]; P[1][x] = C[ca][x]; P[2][x] = C[cb][x]; P[3][x] = C[7][x];
+                }
+                Tet t;
+                finish_tet(P, scale, t);
+                unsigned int tet_id = (unsigned int)(cell * 6 + t6);
+                if (!SCATTER && level == 0) {
+                    long long nc = (long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) *
+                                   (t.hi[2] - t.lo[2] + 1);
+                    atomicAdd(&sh_stat[ST_SUM_CELLS], (unsigned long long)nc);
+                    atomicMax(&sh_stat[ST_MAX_CELLS], (unsigned long long)nc);
+                    atomicAdd(&sh_hist[0][bit_width_u64((unsigned long long)(nc - 1))], 1u);
+                    double det = tet_det(t.g);
+                    if (det < 0.0) atomicAdd(&sh_stat[ST_INVERTED], 1ull);
+                    if (det == 0.0) atomicAdd(&sh_stat[ST_DEGENERATE], 1ull);
+                }
+                for_each_block(t.lo, t.hi, Gl, TILE, nb, [&](int tx, int ty, int tz, long long inside) {
+                    long long id = tile_id_of(s, level, tx, ty, tz);
+                    if (id < 0) return;
+                    if (!SCATTER) {
+                        atomicAdd(&tile_counts[id], 1u);
+                        atomicAdd(&sh_stat[ST_PAIRS], 1ull);
+                        atomicAdd(&sh_hist[1][bit_width_u64((unsigned long long)(inside - 1))], 1u);
+                    } else {
+                        unsigned int slot = atomicAdd(&cursors[id], 1u);
+                        pair_ids[tile_offsets[id] + slot] = tet_id;
+                    }
+                });
+            }
+        }
+    }
+    if (!SCATTER) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < 128; i += blockDim.x) {
+            unsigned int v = (&sh_hist[0][0])[i];
+            if (v) atomicAdd(&hist[i], (unsigned long long)v);
+        }
+        if (threadIdx.x < ST_COUNT && sh_stat[threadIdx.x]) {
+            if (threadIdx.x == ST_MAX_CELLS) atomicMax(&stats[ST_MAX_CELLS], sh_stat[ST_MAX_CELLS]);
+            else atomicAdd(&stats[threadIdx.x], sh_stat[threadIdx.x]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- exclusive scan (3 kernels)
+// in: n uint32 counts -> out: n+1 uint64 exclusive prefix (out[n] = total);
+// second output: items per tile = ceil(count/chunk), scanned the same way.
+constexpr int SCAN_BLOCK = 1024;
+
+__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_partials(const unsigned int* counts, long long n,
+                                                              unsigned int chunk,
+                                                              unsigned long long* part_pairs,
+                                                              unsigned long long* part_items) {
+    __shared__ unsigned long long sp[32], si[32];
+    long long i = blockIdx.x * (long long)SCAN_BLOCK + threadIdx.x;
+    unsigned long long c = i < n ? counts[i] : 0ull;
+    unsigned long long it = (c + chunk - 1) / chunk;
+    for (int o = 16; o; o >>= 1) {
+        c += __shfl_down_sync(0xffffffffu, c, o);
+        it += __shfl_down_sync(0xffffffffu, it, o);
+    }
+    if ((threadIdx.x & 31) == 0) { sp[threadIdx.x >> 5] = c; si[threadIdx.x >> 5] = it; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        c = sp[threadIdx.x]; it = si[threadIdx.x];
+        for (int o = 16; o; o >>= 1) {
+            c += __shfl_down_sync(0xffffffffu, c, o);
+            it += __shfl_down_sync(0xffffffffu, it, o);
+        }
+        if (threadIdx.x == 0) { part_pairs[blockIdx.x] = c; part_items[blockIdx.x] = it; }
+    }
+}
+
+// single block: exclusive scan of the per-block partials in place; totals to totals[0..1]
+__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_top(unsigned long long* part_pairs,
+                                                         unsigned long long* part_items, int nparts,
+                                                         unsigned long long* totals) {
+    __shared__ unsigned long long wp[32], wi[32];
+    __shared__ unsigned long long carry[2];
+    if (threadIdx.x == 0) { carry[0] = 0; carry[1] = 0; }
+    __syncthreads();
+    for (int base = 0; base < nparts; base += SCAN_BLOCK) {
+        int i = base + threadIdx.x;
+        unsigned long long a = i < nparts ? part_pairs[i] : 0ull, b = i < nparts ? part_items[i] : 0ull;
+        unsigned long long ia = a, ib = b;
+        int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+            if (lane >= o) { ia += ta; ib += tb; }
+        }
+        if (lane == 31) { wp[w] = ia; wi[w] = ib; }
+        __syncthreads();
+        if (w == 0) {
+            unsigned long long xa = wp[lane], xb = wi[lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned long long ta = __shfl_up_sync(0xffffffffu, xa, o), tb = __shfl_up_sync(0xffffffffu, xb, o);
+                if (lane >= o) { xa += ta; xb += tb; }
+            }
+            wp[lane] = xa; wi[lane] = xb;
+        }
+        __syncthreads();
+        unsigned long long offa = carry[0] + (w ? wp[w - 1] : 0ull), offb = carry[1] + (w ? wi[w - 1] : 0ull);
+        if (i < nparts) { part_pairs[i] = offa + ia - a; part_items[i] = offb + ib - b; }
+        __syncthreads();
+        if (threadIdx.x == SCAN_BLOCK - 1) { carry[0] = offa + ia; carry[1] = offb + ib; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { totals[0] = carry[0]; totals[1] = carry[1]; }
+}
+
+__global__ void __launch_bounds__(SCAN_BLOCK) k_scan_final(const unsigned int* counts, long long n,
+                                                           unsigned int chunk,
+                                                           const unsigned long long* part_pairs,
+                                                           const unsigned long long* part_items,
+                                                           unsigned long long* tile_offsets,
+                                                           unsigned long long* item_offsets) {
+    __shared__ unsigned long long wp[32], wi[32];
+    long long i = blockIdx.x * (long long)SCAN_BLOCK + threadIdx.x;
+    unsigned long long a = i < n ? counts[i] : 0ull;
+    unsigned long long b = (a + chunk - 1) / chunk;
+    unsigned long long ia = a, ib = b;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+        if (lane >= o) { ia += ta; ib += tb; }
+    }
+    if (lane == 31) { wp[w] = ia; wi[w] = ib; }
+    __syncthreads();
+    if (w == 0) {
+        unsigned long long xa = wp[lane], xb = wi[lane];
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long ta = __shfl_up_sync(0xffffffffu, xa, o), tb = __shfl_up_sync(0xffffffffu, xb, o);
+            if (lane >= o) { xa += ta; xb += tb; }
+        }
+        wp[lane] = xa; wi[lane] = xb;
+    }
+    __syncthreads();
+    unsigned long long offa = part_pairs[blockIdx.x] + (w ? wp[w - 1] : 0ull);
+    unsigned long long offb = part_items[blockIdx.x] + (w ? wi[w - 1] : 0ull);
+    if (i < n) { tile_offsets[i] = offa + ia - a; item_offsets[i] = offb + ib - b; }
+    if (i == n - 1) { tile_offsets[n] = offa + ia; item_offsets[n] = offb + ib; }
+}
+
+// work items: each tile's pair list cut into chunks
+__global__ void k_items(const unsigned int* counts, long long n, unsigned int chunk,
+                        const unsigned long long* tile_offsets,
+                        const unsigned long long* item_offsets, Item* items) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    unsigned int c = counts[t];
+    unsigned long long io = item_offsets[t], po = tile_offsets[t];
+    for (unsigned int done = 0; done < c; done += chunk) {
+        Item it;
+        it.tile = (unsigned int)t;
+        it.count = min(chunk, c - done);
+        it.begin = po + done;
+        items[io++] = it;
+    }
+}
+
+// ---------------------------------------------------------------- a4-a6 binned deposit
+struct DepositArgs {
+    Particles part;
+    Space space;
+    const unsigned int* pair_ids;
+    const Item* items;
+    double mass_per_tet;
+    int weight_mode;  // 0 mass, 1 signed volume
+    int chord_axis;   // -1 adaptive, else 0..2
+    unsigned long long* stats;
+};
+
+constexpr int DEP_WARPS = 4;
+constexpr int DEP_THREADS = DEP_WARPS * 32;
+// per-warp scratch in doubles: tet slots [13][32] + polygon [24][32] + chord planes [9][32]
+constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP + 9) * 32;
+constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
+
+__device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile, int& level,
+                                              int org[3], double*& out, long long str[3]) {
+    if (!s.patch_mode) {
+        int tz = tile % s.nt, ty = (tile / s.nt) % s.nt, tx = tile / (s.nt * s.nt);
+        level = 0;
+        org[0] = tx * TILE; org[1] = ty * TILE; org[2] = tz * TILE;
+        str[0] = (long long)s.G * s.G; str[1] = s.G; str[2] = 1;
+        out = s.out + org[0] * str[0] + org[1] * str[1] + org[2];
+    } else {
+        int tp3 = s.tp * s.tp * s.tp;
+        unsigned int pi = tile / tp3, sub = tile % tp3;
+        PatchDev pd = s.patches[pi];
+        int sz = sub % s.tp, sy = (sub / s.tp) % s.tp, sx = sub / (s.tp * s.tp);
+        level = pd.level;
+        org[0] = pd.ox * s.P + sx * TILE; org[1] = pd.oy * s.P + sy * TILE; org[2] = pd.oz * s.P + sz * TILE;
+        str[0] = (long long)s.P * s.P; str[1] = s.P; str[2] = 1;
+        out = s.out + (long long)pi * s.P * s.P * s.P + (sx * TILE) * str[0] + (sy * TILE) * str[1] + sz * TILE;
+    }
+}
+
+template <bool COUNT>
+__global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A) {
+    extern __shared__ double smem[];
+    double* acc = smem;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;  // [13][32]
+    double* wpoly = wtet + 13 * 32;                          // [24][32]
+    double* wrt = wpoly + 3 * POLY_CAP * 32;                 // [9][32]
+    PolyBuf<32> poly{wpoly + lane};
+    double* rt = wrt + lane;
+
+    const Item item = A.items[blockIdx.x];
+    int level, org[3];
+    double* out;
+    long long str[3];
+    tile_geometry(A.space, item.tile, level, org, out, str);
+    const double scale = level_scale(A.space, level);
+    const int Gl = level_G(A.space, level);
+
+    for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
+    __syncthreads();
+
+    ColumnCounters cnt = {0, 0, 0, 0};
+
+    for (unsigned int base = warp * 32; base < item.count; base += DEP_WARPS * 32) {
+        // ---- a1: each lane builds one tet of the batch
+        const bool have = base + lane < item.count;
+        Tet t;
+        double det = 1.0;
+        int nimg[3] = {1, 1, 1}, mlo[3] = {0, 0, 0};
+        if (have) {
+            unsigned int id = A.pair_ids[item.begin + base + lane];
+            double P[4][3];
+            load_tet_vertices(A.part, id / 6, id % 6, P);
+            finish_tet(P, scale, t);
+            det = tet_det(t.g);
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {  // periodic images of this tile met by the tet's range
+                mlo[x] = -floor_div(org[x] + TILE - 1 - t.lo[x], Gl);
+                nimg[x] = floor_div(t.hi[x] - org[x], Gl) - mlo[x] + 1;
+            }
+        }
+        int my_images = have ? nimg[0] * nimg[1] * nimg[2] : 0;
+        const int max_images = __reduce_max_sync(0xffffffffu, my_images);
+        for (int img = 0; img < max_images; ++img) {
+            // ---- slot setup: tile-local vertices, weight, column range
+            int info = 0, ncol = 0;
+            __syncwarp();
+            if (img < my_images) {
+                int m[3] = {mlo[0] + img % nimg[0], mlo[1] + (img / nimg[0]) % nimg[1],
+                            mlo[2] + img / (nimg[0] * nimg[1])};
+                int lo[3], hi[3];
+#pragma unroll
+                for (int x = 0; x < 3; ++x) {
+                    int o = org[x] + m[x] * Gl;
+                    lo[x] = max(t.lo[x] - o, 0);
+                    hi[x] = min(t.hi[x] - o, TILE - 1);
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) wtet[(3 * v + x) * 32 + lane] = t.g[v][x] - (double)o;
+                }
+                double w;
+                if (A.weight_mode == 0) w = det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0;
+                else w = 1.0;
+                wtet[12 * 32 + lane] = w;
+                int ax = A.chord_axis;
+                if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
+                    int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
+                    ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
+                }
+                int av = (ax + 1) % 3, aw = (ax + 2) % 3;
+                ncol = (hi[av] - lo[av] + 1) * (hi[aw] - lo[aw] + 1);
+                if (det == 0.0) {  // degenerate: whole mass to the centroid cell (Q6)
+                    ncol = 0;
+                    if (A.weight_mode == 0) {
+                        int c[3];
+                        bool in = true;
+#pragma unroll
+                        for (int x = 0; x < 3; ++x) {
+                            double cen = (t.g[0][x] + t.g[1][x] + t.g[2][x] + t.g[3][x]) / 4.0;
+                            c[x] = __double2int_rd(cen) - (org[x] + m[x] * Gl);
+                            in = in && c[x] >= 0 && c[x] < TILE;
+                        }
+                        if (in) atomicAdd(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], A.mass_per_tet);
+                    }
+                }
+                info = lo[ax] | (hi[ax] << 3) | lo[av] << 6 | (hi[av] - lo[av]) << 9 | lo[aw] << 12 |
+                       (hi[aw] - lo[aw]) << 15 | ax << 18;
+            }
+            // ---- exclusive prefix of column counts over the 32 slots
+            int pre = ncol;
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, pre, o);
+                if (lane >= o) pre += y;
+            }
+            const int total = __shfl_sync(0xffffffffu, pre, 31);
+            pre -= ncol;
+            __syncwarp();
+            // ---- a4-a6: columns of all 32 tets spread evenly over the lanes
+            for (int cb = 0; cb < total; cb += 32) {
+                const int cand = cb + lane;
+                int slot = 0;  // largest slot with pre[slot] <= cand
+#pragma unroll
+                for (int step = 16; step; step >>= 1) {
+                    int probe = __shfl_sync(0xffffffffu, pre, slot + step);
+                    if (probe <= cand) slot += step;
+                }
+                const int sinfo = __shfl_sync(0xffffffffu, info, slot);
+                const int spre = __shfl_sync(0xffffffffu, pre, slot);
+                if (cand < total) {
+                    const int a0 = sinfo & 7, a1 = (sinfo >> 3) & 7;
+                    const int v0 = (sinfo >> 6) & 7, w0 = (sinfo >> 12) & 7;
+                    const int nw = ((sinfo >> 15) & 7) + 1;
+                    const int ax = (sinfo >> 18) & 3;
+                    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
+                    const int local = cand - spre;
+                    const int cv = v0 + local / nw, cw = w0 + local % nw;
+                    const double* ts = wtet + slot;
+                    const double ou = (double)a0, ov = (double)cv, ow = (double)cw;
+                    auto getv = [&](int vi, int comp) -> double {
+                        int axis = comp == 0 ? ax : (comp == 1 ? av : aw);
+                        double off = comp == 0 ? ou : (comp == 1 ? ov : ow);
+                        return ts[(3 * vi + axis) * 32] - off;
+                    };
+                    const double w = ts[12 * 32];
+                    // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
+                    const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
+                    const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
+                    const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
+                    double* col = acc + a0 * su + cv * sv + cw * sw;
+                    column_task<32, COUNT>(getv, a1 - a0 + 1, poly, rt,
+                                           [&](int c, double val) { atomicAdd(col + c * su, w * val); },
+                                           &cnt);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // ---- a6: flush the tile with fp64 reductions (other work items may hold the same tile)
+    for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) {
+        double v = acc[i];
+        if (v != 0.0) {
+            int cz = i & 7, cy = (i >> 3) & 7, cx = i >> 6;
+            atomicAdd(out + cx * str[0] + cy * str[1] + cz, v);
+        }
+    }
+    if (COUNT) {
+        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.tasks), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
+        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_clips), d = __reduce_add_sync(0xffffffffu, cnt.cells);
+        if (lane == 0) {
+            atomicAdd(&A.stats[ST_TASKS], (unsigned long long)a);
+            atomicAdd(&A.stats[ST_FACE_CLIPS], (unsigned long long)b);
+            atomicAdd(&A.stats[ST_PLANE_CLIPS], (unsigned long long)c);
+            atomicAdd(&A.stats[ST_CELLS], (unsigned long long)d);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- direct path (any G)
+// One thread per tet, polygon in local memory, global fp64 atomics with periodic wrap.
+// The plain first path: kept as PSD_OPT_KERNEL = 1 and for grids the tiling does not divide.
+template <bool COUNT>
+__global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
+    const int64_t ntet = (int64_t)6 * A.part.N * A.part.N * A.part.N;
+    int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    ColumnCounters cnt = {0, 0, 0, 0};
+    if (id < ntet) {
+        const Space& s = A.space;
+        const int G = s.G;
+        double P[4][3];
+        load_tet_vertices(A.part, id / 6, (int)(id % 6), P);
+        Tet t;
+        finish_tet(P, level_scale(s, 0), t);
+        double det = tet_det(t.g);
+        if (det == 0.0) {
+            if (A.weight_mode == 0) {
+                int c[3];
+#pragma unroll
+                for (int x = 0; x < 3; ++x)
+                    c[x] = wrap_mod(__double2int_rd((t.g[0][x] + t.g[1][x] + t.g[2][x] + t.g[3][x]) / 4.0), G);
+                atomicAdd(&s.out[((long long)c[0] * G + c[1]) * G + c[2]], A.mass_per_tet);
+            }
+        } else {
+            const double w = A.weight_mode == 0 ? 6.0 * A.mass_per_tet / det : 1.0;
+            double polymem[3 * POLY_CAP], rtmem[9];
+            PolyBuf<1> poly{polymem};
+            int ax = A.chord_axis;
+            if (ax < 0) {
+                int e0 = t.hi[0] - t.lo[0], e1 = t.hi[1] - t.lo[1], e2 = t.hi[2] - t.lo[2];
+                ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
+            }
+            const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
+            for (int cv = t.lo[av]; cv <= t.hi[av]; ++cv)
+                for (int cw = t.lo[aw]; cw <= t.hi[aw]; ++cw)
+                    for (int u0 = t.lo[ax]; u0 <= t.hi[ax]; u0 += TILE) {
+                        int na = min(TILE, t.hi[ax] - u0 + 1);
+                        auto getv = [&](int vi, int comp) -> double {
+                            int axis = comp == 0 ? ax : (comp == 1 ? av : aw);
+                            double off = comp == 0 ? (double)u0 : (comp == 1 ? (double)cv : (double)cw);
+                            // dynamic index into t.g: local memory, fine for this path
+                            return t.g[vi][axis] - off;
+                        };
+                        column_task<1, COUNT>(getv, na, poly, rtmem, [&](int c, double val) {
+                            int cc[3];
+                            cc[ax] = wrap_mod(u0 + c, G); cc[av] = wrap_mod(cv, G); cc[aw] = wrap_mod(cw, G);
+                            atomicAdd(&s.out[((long long)cc[0] * G + cc[1]) * G + cc[2]], w * val);
+                        }, &cnt);
+                    }
+        }
+    }
+    if (COUNT) {
+        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.tasks), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
+        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_clips), d = __reduce_add_sync(0xffffffffu, cnt.cells);
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(&A.stats[ST_TASKS], (unsigned long long)a);
+            atomicAdd(&A.stats[ST_FACE_CLIPS], (unsigned long long)b);
+            atomicAdd(&A.stats[ST_PLANE_CLIPS], (unsigned long long)c);
+            atomicAdd(&A.stats[ST_CELLS], (unsigned long long)d);
+        }
+    }
+}
+
+// census-only statistics for the direct path (no tiles): sum/max cells, histogram, inverted
+__global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, unsigned long long* stats,
+                                                   unsigned long long* hist) {
+    int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
+    int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (id >= ntet) return;
+    double P[4][3];
+    load_tet_vertices(p, id / 6, (int)(id % 6), P);
+    Tet t;
+    finish_tet(P, scale, t);
+    long long nc = (long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) * (t.hi[2] - t.lo[2] + 1);
+    atomicAdd(&stats[ST_SUM_CELLS], (unsigned long long)nc);
+    atomicMax(&stats[ST_MAX_CELLS], (unsigned long long)nc);
+    atomicAdd(&hist[bit_width_u64((unsigned long long)(nc - 1))], 1ull);
+    double det = tet_det(t.g);
+    if (det < 0.0) atomicAdd(&stats[ST_INVERTED], 1ull);
+    if (det == 0.0) atomicAdd(&stats[ST_DEGENERATE], 1ull);
+}
+
+// ---------------------------------------------------------------- a7 refinement census
+// counts[level] (dense, (base_G/P * 2^level)^3): tets whose cell range on the level grid meets
+// each candidate patch position, each position once per tet.
+__global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, int P, int level,
+                                                      unsigned long long* counts) {
+    int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
+    int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (id >= ntet) return;
+    const int Gl = base_G << level;
+    const int np = Gl / P;
+    double V[4][3];
+    load_tet_vertices(p, id / 6, (int)(id % 6), V);
+    Tet t;
+    finish_tet(V, __ddiv_rn((double)Gl, p.L), t);
+    for_each_block(t.lo, t.hi, Gl, P, np, [&](int bx, int by, int bz, long long) {
+        atomicAdd(&counts[((long long)bx * np + by) * np + bz], 1ull);
+    });
+}
+
+}  // namespace psd
