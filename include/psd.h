@@ -28,6 +28,12 @@
 
 #include <stdint.h>
 
+#if defined(__GNUC__)
+#define PSD_API __attribute__((visibility("default")))
+#else
+#define PSD_API
+#endif
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -95,10 +101,10 @@ typedef struct {
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the
  * legacy default stream) that all work of this context is enqueued on; it must outlive
  * the context. */
-int psd_create(psd_ctx** out, int device, void* cuda_stream);
+PSD_API int psd_create(psd_ctx** out, int device, void* cuda_stream);
 
 /* Frees only context-owned scratch.  NULL is allowed. */
-void psd_destroy(psd_ctx* ctx);
+PSD_API void psd_destroy(psd_ctx* ctx);
 
 /* PAPER.md:39-45, :60.  Register the particle set the tets are generated from.
  *   pos_dev      N^3 particles in Lagrangian order: particle (i,j,k) at element offset
@@ -112,7 +118,7 @@ void psd_destroy(psd_ctx* ctx);
  * cell's corner 0; valid while every cell edge is shorter than L/2): nothing is stored.
  * Runs one validation pass over the positions and synchronises; non-finite positions give
  * PSD_ERR_INVALID_ARG. */
-int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elems, int N, double L,
+PSD_API int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elems, int N, double L,
                    double total_mass);
 
 /* PAPER.md:137, :155-161.  Deposit all 6 N^3 tets onto the uniform periodic grid.
@@ -120,7 +126,7 @@ int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elem
  *   grid_dev   G^3 doubles, index (ix*G+iy)*G+iz, MASS per cell (not density).
  *   accumulate 0: the library zeroes the grid first; 1: adds to what is there.
  * Asynchronous. */
-int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate);
+PSD_API int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate);
 
 /* PAPER.md:66 (refinement by tet count), :72 (leaf patches).  Census-driven construction of
  * the patch list: counts, per level l = 0..max_level, the tets whose cell range meets each
@@ -131,7 +137,7 @@ int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate);
  *   counts_host  optional: receives the dense count arrays of all levels, concatenated
  *                (sum over l of (base_G/P * 2^l)^3 uint64)
  * Synchronous. */
-int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
+PSD_API int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
                        psd_patch* out_host, int64_t cap, int64_t* n_out, uint64_t* counts_host);
 
 /* PAPER.md:72, Q13.  Deposit into every listed patch the full contribution of
@@ -140,27 +146,33 @@ int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double fa
  *   P             cells per patch side, multiple of 8;  base_G % P == 0
  *   mass_dev      n_patch * P^3 doubles, patch-major then (x*P+y)*P+z
  * Asynchronous (the patch list is copied before return). */
-int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_patch, int P,
+PSD_API int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_patch, int P,
                         int base_G, double* mass_dev, int accumulate);
 
 /* End-to-end convenience used for the host-buffer measurement: copies positions host->device,
  * registers them, deposits, copies the G^3 grid device->host.  Synchronous.  Host buffers
  * should be pinned for full copy bandwidth. */
-int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
+PSD_API int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
                              double L, double total_mass, int G, double* grid_host);
 
 /* Synchronises, then fills *out with the counters of the last build / deposit. */
-int psd_get_stats(psd_ctx* ctx, psd_stats* out);
+PSD_API int psd_get_stats(psd_ctx* ctx, psd_stats* out);
 
-int psd_set_option(psd_ctx* ctx, int key, double value);
-int psd_sync(psd_ctx* ctx);
-const char* psd_last_error(const psd_ctx* ctx);
+/* Synchronises, then copies the per-tile (tet, tile) pair counts of the last binned deposit to
+ * out_host (n_tiles uint32; cap = its capacity in elements).  Uniform grid: tile
+ * (tx*nt+ty)*nt+tz, nt = G/8.  Patches: patch-major, then the (P/8)^3 tiles of the patch.
+ * PSD_ERR_STATE if the last deposit was not binned. */
+PSD_API int psd_get_tile_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap);
+
+PSD_API int psd_set_option(psd_ctx* ctx, int key, double value);
+PSD_API int psd_sync(psd_ctx* ctx);
+PSD_API const char* psd_last_error(const psd_ctx* ctx);
 
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
-int64_t psd_launch_count(const psd_ctx* ctx);
+PSD_API int64_t psd_launch_count(const psd_ctx* ctx);
 
 /* Library identification: "libpsd sm_100a <build date>" */
-const char* psd_version(void);
+PSD_API const char* psd_version(void);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,11 @@
+"""paper_1612_09491_b200 -- B200 (sm_100a) phase-space-element mass deposit (arXiv:1612.09491).
+
+The product is the C-ABI CUDA library `libpsd.so` (include/psd.h); this package is its thin
+ctypes binding (argument marshalling only).  There is no CPU fallback: importing the binding
+without the built library, or creating a context without a CUDA device, fails loudly.
+"""
+from .binding import (  # noqa: F401
+    F32, F64, OPT_WEIGHT_MODE, OPT_KERNEL, OPT_COUNTERS, OPT_CHUNK, OPT_CHORD_AXIS,
+    RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN, PsdError, PsdStats, Context, lib, version,
+    EXPORTS,
+)

@@ -41,7 +41,7 @@ struct psd_ctx {
     Particles part{};
     bool built = false;
     double total_mass = 0.0;
-    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = 0;
+    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1;
     unsigned int chunk = 1024;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
         totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid;
@@ -496,6 +496,17 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
         CK(cudaStreamSynchronize(ctx->stream));
     }
     *out = ctx->last;
+    return PSD_OK;
+}
+
+int psd_get_tile_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap) {
+    if (!valid_ctx(ctx) || !out_host) return PSD_ERR_INVALID_ARG;
+    if (!ctx->binned_last || ctx->last.n_tiles <= 0) return fail(ctx, PSD_ERR_STATE, "no binned deposit to report");
+    if (cap < ctx->last.n_tiles) return fail(ctx, PSD_ERR_INVALID_ARG, "tile count buffer too small");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(out_host, ctx->tile_counts.p, sizeof(uint32_t) * (size_t)ctx->last.n_tiles,
+                       cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
     return PSD_OK;
 }
 

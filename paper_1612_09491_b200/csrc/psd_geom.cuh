@@ -294,7 +294,10 @@ __device__ __forceinline__ void column_task(GetV getv, int na, PolyBuf<S> q, dou
             maxu = fmax(maxu, u);
         }
         // no area inside the column, or entirely below the first plane: contributes nothing
-        if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0 || maxu <= 0.0) continue;
+        if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) continue;
+        // a face below the first plane adds nothing to any R(a), but the tet may reach down to it:
+        // the run of cells then starts at cell 0
+        if (maxu <= 0.0) { col_min = fmin(col_min, 0.0); continue; }
         int n = 3;
         if (minv < 0.0) n = clip_wall<S, 1, 0>(q, n);
         if (maxv > 1.0) n = clip_wall<S, 1, 1>(q, n);
@@ -315,7 +318,7 @@ __device__ __forceinline__ void column_task(GetV getv, int na, PolyBuf<S> q, dou
             umin = fmin(umin, cu); umax = fmax(umax, cu);
             lu = cu; lv = cv; lw = cw;
         }
-        if (umax <= 0.0) continue;
+        if (umax <= 0.0) { col_min = fmin(col_min, 0.0); continue; }
         col_min = fmin(col_min, umin); col_max = fmax(col_max, umax);
         double A = 0.5 * A2, M1 = M6 * (1.0 / 6.0);
         for (int a = 0; a <= na; ++a) {

@@ -1,0 +1,328 @@
+"""GPU parity: the CUDA path (through the C ABI, include/psd.h) against the CPU oracle on the
+same seeded inputs.  Tolerances are BASELINE.json's north_star:
+    per cell |gpu - oracle| <= 1e-9 * max_cell + 1e-6 * |oracle|
+    total mass within 1e-10 relative
+    tet and bin counts bit-exact.
+"""
+import numpy as np
+import pytest
+
+import psd_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def psd():
+    import paper_1612_09491_b200 as m
+    return m
+
+
+@pytest.fixture()
+def ctx(psd):
+    c = psd.Context(0)
+    yield c
+    c.close()
+
+
+def to_dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def assert_parity(gpu, ora, M=1.0, what=""):
+    gpu = np.asarray(gpu).reshape(ora.shape)
+    mx = float(ora.max())
+    err = np.abs(gpu - ora)
+    bound = 1e-9 * mx + 1e-6 * np.abs(ora)
+    worst = float((err / bound).max())
+    assert worst <= 1.0, f"{what}: worst |err|/bound = {worst:.3e}, max |err| = {err.max():.3e}"
+
+
+def assert_mass(gpu_sum, M=1.0):
+    assert abs(float(gpu_sum) - M) <= 1e-10 * abs(M), f"mass {float(gpu_sum)!r} vs {M}"
+
+
+def crossing_field(N, rms, seed=7, dtype="float64", stride=3, modes=24, kmax=3):
+    return psd_inputs.zeldovich_positions(N, modes, kmax, rms, seed, dtype=dtype, stride=stride)
+
+
+KERNELS = [0, 1]  # 0 = binned tile path, 1 = direct path
+
+
+# ------------------------------------------------------------------ invariants on the GPU alone
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("N,G,shift", [(4, 8, (0, 0, 0)), (4, 8, (0.013, 0.4, 0.77)),
+                                       (6, 16, (0.1, 0.2, 0.3)), (5, 9, (0.1, 0.2, 0.3)),
+                                       (8, 8, (0.5, 0.25, 0.125)), (3, 24, (0.01, 0.02, 0.03))])
+def test_unperturbed_lattice_is_uniform(psd, ctx, kernel, N, G, shift):
+    ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+    ctx.psd_build_tets(to_dev(psd_inputs.lattice(N, shift=shift)), 1.0, 2.5)
+    g = ctx.psd_deposit_uniform(G).cpu().numpy()
+    assert np.allclose(g, 2.5 / G ** 3, rtol=1e-11, atol=0)
+    s = ctx.psd_get_stats()
+    assert s.n_tets == 6 * N ** 3 and s.n_inverted == 0 and s.n_degenerate == 0
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_sheared_torus_is_uniform(psd, ctx, kernel):
+    ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+    ctx.psd_build_tets(to_dev(psd_inputs.lattice(6, shift=(0.21, 0.05, 0.6), shear_xy=1)))
+    g = ctx.psd_deposit_uniform(16).cpu().numpy()
+    assert np.allclose(g, 1.0 / 16 ** 3, rtol=1e-11, atol=0)
+
+
+# ------------------------------------------------------------------ element-by-element parity
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("N,G,rms", [(12, 24, 2.0), (12, 8, 2.0), (10, 40, 1.0), (16, 64, 3.0),
+                                     (6, 72, 0.5)])
+def test_crossing_field_parity(psd, ctx, oracle, kernel, N, G, rms):
+    """Heavily multistream small fields: inverted tets, tets spanning several tiles, tiles met
+    through two periodic images (G = 8 with 2-cell-rms displacements)."""
+    pos = crossing_field(N, rms)
+    ora, st = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(G)
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora, what=f"N{N} G{G}")
+    s = ctx.psd_get_stats()
+    assert s.n_inverted == st["n_inverted"] and s.sum_cells == st["n_candidates"]
+    # signed-volume mode: every cell exactly one cell volume for any displacement field
+    ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
+    sg = ctx.psd_deposit_uniform(G).cpu().numpy()
+    assert np.allclose(sg, 1.0, rtol=0, atol=1e-10)
+
+
+@pytest.mark.parametrize("G", [9, 20, 63])
+def test_ragged_grid_sizes_use_direct_path(psd, ctx, oracle, G):
+    """G not a multiple of the tile edge (Q12)."""
+    pos = crossing_field(8, 1.2, seed=3)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(G)
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora)
+    assert ctx.psd_get_stats().n_tiles == 0
+
+
+@pytest.mark.parametrize("chord_axis", [-1, 0, 1, 2])
+def test_chord_axis_choices_agree(psd, ctx, oracle, chord_axis):
+    pos = crossing_field(10, 1.5, seed=11)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 32)
+    ctx.psd_set_option(psd.OPT_CHORD_AXIS, chord_axis)
+    ctx.psd_build_tets(to_dev(pos))
+    assert_parity(ctx.psd_deposit_uniform(32).cpu().numpy(), ora)
+
+
+@pytest.mark.parametrize("dtype,stride", [("float32", 4), ("float32", 3), ("float64", 3), ("float64", 4)])
+def test_position_layouts(psd, ctx, oracle, dtype, stride):
+    pos = crossing_field(9, 1.0, dtype=dtype, stride=stride)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 24)
+    ctx.psd_build_tets(to_dev(pos))
+    assert_parity(ctx.psd_deposit_uniform(24).cpu().numpy(), ora)
+
+
+def test_box_length_total_mass_and_accumulate(psd, ctx, oracle):
+    pos = crossing_field(8, 0.9) * 3.0
+    ora, _ = oracle.deposit_uniform(pos, 3.0, 7.0, 16)
+    ctx.psd_build_tets(to_dev(pos), 3.0, 7.0)
+    g = ctx.psd_deposit_uniform(16)
+    assert_mass(g.sum(), 7.0)
+    assert_parity(g.cpu().numpy(), ora)
+    ctx.psd_deposit_uniform(16, g, accumulate=True)
+    assert_parity(g.cpu().numpy(), 2.0 * ora)
+
+
+def test_degenerate_all_coincident(psd, ctx, oracle):
+    """Q6: V = 0 exactly -> the whole tet mass goes to the centroid cell."""
+    pos = np.full((4, 4, 4, 3), 0.3, dtype=np.float64)
+    ora, st = oracle.deposit_uniform(pos, 1.0, 1.0, 8)
+    for kernel in KERNELS:
+        ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+        ctx.psd_build_tets(to_dev(pos))
+        g = ctx.psd_deposit_uniform(8).cpu().numpy()
+        assert ctx.psd_get_stats().n_degenerate == st["n_degenerate"] == 6 * 64
+        assert_parity(g, ora)
+
+
+def test_cfg0_full_parity_and_bit_exact_census(psd, ctx, oracle):
+    """BASELINE.json configs[0]: 32^3 particles, fp64, 64^3 grid, every cell compared."""
+    pos = psd_inputs.config_positions(0)
+    ora, st = oracle.deposit_uniform(pos, 1.0, 1.0, 64)
+    cen = oracle.census(pos, 1.0, 64)
+    assert st["n_inverted"] == 0
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(64)
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora, what="cfg0")
+    s = ctx.psd_get_stats()
+    assert s.n_tets == cen["n_tets"] == 196608
+    assert s.n_pairs == cen["n_pairs"] and s.sum_cells == cen["sum_cells"]
+    assert s.max_cells == cen["max_cells"] and s.n_inverted == 0
+    assert list(s.hist_tet) == cen["hist_tet"].tolist()
+    assert list(s.hist_pair) == cen["hist_pair"].tolist()
+    assert np.array_equal(ctx.psd_get_tile_counts(), cen["tile_counts"])
+    ctx.psd_set_option(psd.OPT_KERNEL, 1)
+    assert_parity(ctx.psd_deposit_uniform(64).cpu().numpy(), ora, what="cfg0 direct")
+
+
+def test_census_bit_exact_with_images_and_inversions(psd, ctx, oracle):
+    pos = crossing_field(12, 2.0, dtype="float32", stride=4)
+    for G in (8, 24, 48):
+        cen = oracle.census(pos, 1.0, G)
+        ctx.psd_build_tets(to_dev(pos))
+        ctx.psd_deposit_uniform(G)
+        s = ctx.psd_get_stats()
+        assert (s.n_pairs, s.sum_cells, s.max_cells, s.n_inverted) == (
+            cen["n_pairs"], cen["sum_cells"], cen["max_cells"], cen["n_inverted"])
+        assert list(s.hist_tet) == cen["hist_tet"].tolist()
+        assert list(s.hist_pair) == cen["hist_pair"].tolist()
+        assert np.array_equal(ctx.psd_get_tile_counts(), cen["tile_counts"])
+
+
+@pytest.mark.parametrize("chunk", [32, 100, 1024])
+def test_work_item_chunking_does_not_change_the_result(psd, ctx, oracle, chunk):
+    pos = crossing_field(12, 2.0)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 16)
+    ctx.psd_set_option(psd.OPT_CHUNK, chunk)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(16)
+    assert_parity(g.cpu().numpy(), ora)
+    s = ctx.psd_get_stats()
+    tc = ctx.psd_get_tile_counts().astype(np.int64)
+    assert s.n_work_items == int(((tc + chunk - 1) // chunk).sum())
+
+
+# ------------------------------------------------------------------ patch path
+def test_patches_parity_and_refinement(psd, ctx, oracle):
+    """a7: refinement census bit-exact, rule reproduces the oracle's list, deposit parity on
+    every level, level 0 tiled = uniform deposit, coarse cell = sum of its 8 children."""
+    pos = crossing_field(16, 2.5, dtype="float32", stride=4, modes=40, kmax=4)
+    base_G, P, max_level, factor = 32, 16, 2, 1.5
+    ctx.psd_build_tets(to_dev(pos))
+    patches, counts = ctx.psd_refine_patches(base_G, P, max_level, factor, want_counts=True)
+    ocounts = [oracle.patch_counts(pos, 1.0, base_G, P, l) for l in range(max_level + 1)]
+    for a, b in zip(counts, ocounts):
+        assert np.array_equal(a, b)
+    opatches = oracle.refine_patches(ocounts, factor)
+    assert np.array_equal(patches, opatches)
+    assert (patches[:, 0] == 1).any() and (patches[:, 0] == 2).any()
+    lit = ctx.psd_refine_patches(base_G, P, max_level, factor, rule=psd.RULE_LITERAL_TOP_DOWN)
+    assert np.array_equal(lit, oracle.refine_patches(ocounts, factor, oracle.RULE_LITERAL_TOP_DOWN))
+    ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches)
+    mass = ctx.psd_deposit_patches(patches, P, base_G).cpu().numpy()
+    mx = ora.max()
+    assert (np.abs(mass - ora) <= 1e-9 * mx + 1e-6 * np.abs(ora)).all()
+    # level 0 tiled together == uniform deposit at base_G (Q13)
+    uni = ctx.psd_deposit_uniform(base_G).cpu().numpy()
+    l0 = patches[:, 0] == 0
+    for row, m in zip(patches[l0], mass[l0]):
+        _, ox, oy, oz = row
+        blk = uni[ox * P:(ox + 1) * P, oy * P:(oy + 1) * P, oz * P:(oz + 1) * P]
+        assert np.allclose(m, blk, rtol=1e-9, atol=1e-15)
+    assert_mass(mass[l0].sum())
+
+
+def test_patch_list_subset_and_order_independence(psd, ctx, oracle):
+    pos = crossing_field(12, 2.0)
+    patches = np.array([[1, 3, 0, 2], [0, 1, 1, 0], [2, 7, 7, 7], [0, 0, 0, 1], [1, 0, 3, 3]], dtype=np.int32)
+    ora = oracle.deposit_patches(pos, 1.0, 1.0, 32, 16, patches)
+    ctx.psd_build_tets(to_dev(pos))
+    mass = ctx.psd_deposit_patches(patches, 16, 32).cpu().numpy()
+    assert (np.abs(mass - ora) <= 1e-9 * ora.max() + 1e-6 * np.abs(ora)).all()
+    perm = np.array([4, 2, 0, 3, 1])
+    mass2 = ctx.psd_deposit_patches(patches[perm], 16, 32).cpu().numpy()
+    assert np.allclose(mass2, mass[perm], rtol=1e-9, atol=1e-18)
+
+
+# ------------------------------------------------------------------ boundary behaviour
+def test_error_codes(psd, ctx):
+    import torch
+    with pytest.raises(psd.PsdError) as e:
+        ctx.psd_deposit_uniform(8)
+    assert e.value.code == 2  # PSD_ERR_STATE
+    bad = torch.full((4, 4, 4, 3), float("nan"), dtype=torch.float64, device="cuda")
+    with pytest.raises(psd.PsdError) as e:
+        ctx.psd_build_tets(bad)
+    assert e.value.code == 1
+    ctx.psd_build_tets(to_dev(psd_inputs.lattice(4)))
+    with pytest.raises(psd.PsdError):
+        ctx._ck(ctx._L.psd_deposit_uniform(ctx._h, 0, 0, 0))
+    with pytest.raises(psd.PsdError):
+        ctx.psd_set_option(99, 1)
+    with pytest.raises(psd.PsdError):
+        ctx.psd_deposit_patches(np.array([[0, 5, 0, 0]], dtype=np.int32), 16, 32)  # origin outside
+    with pytest.raises(psd.PsdError):
+        ctx.psd_deposit_patches(np.array([[0, 0, 0, 0], [0, 0, 0, 0]], dtype=np.int32), 16, 32)
+    # the context still works after errors
+    g = ctx.psd_deposit_uniform(8).cpu().numpy()
+    assert np.allclose(g, 1.0 / 512, rtol=1e-12)
+
+
+def test_host_buffer_entry_point(psd, ctx, oracle):
+    import torch
+    pos = crossing_field(10, 1.0, dtype="float32", stride=4)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 24)
+    hp = torch.from_numpy(pos).pin_memory()
+    hg = torch.empty((24, 24, 24), dtype=torch.float64).pin_memory()
+    ctx.psd_deposit_uniform_host(hp, 24, hg)
+    assert_parity(hg.numpy(), ora)
+    assert ctx.psd_launch_count() > 0
+
+
+def test_runs_on_a_non_default_stream(psd, oracle):
+    import torch
+    pos = crossing_field(10, 1.0)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 16)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        d = to_dev(pos)
+    st.synchronize()
+    c = psd.Context(0, stream=st)
+    c.psd_build_tets(d)
+    g = c.psd_deposit_uniform(16)
+    c.psd_sync()
+    assert_parity(g.cpu().numpy(), ora)
+    c.close()
+
+
+# ------------------------------------------------------------------ full-size configs
+def sample_windows(G, n, edge, seed):
+    u = psd_inputs.splitmix64(seed, 0, 3 * n) % np.uint64(G)
+    return [tuple(int(x) for x in u[3 * i:3 * i + 3]) for i in range(n)], edge
+
+
+def window_of(grid_dev, lo, edge, G):
+    import torch
+    ix = [(torch.arange(edge, device=grid_dev.device) + l) % G for l in lo]
+    return grid_dev[ix[0]][:, ix[1]][:, :, ix[2]].cpu().numpy()
+
+
+@pytest.mark.parametrize("cfg_index,n_win,edge", [(1, 6, 12), (2, 3, 10)])
+def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_win, edge):
+    """BASELINE.json configs[1], [2] at full size in the launch configuration bench.py times:
+    total mass, signed-volume cover of every cell, and oracle parity on sampled windows
+    (windows may wrap around the box)."""
+    import torch
+    cfg = psd_inputs.CONFIGS[cfg_index]
+    G = cfg["G"]
+    pos = psd_inputs.config_positions(cfg_index)
+    ctx.psd_build_tets(to_dev(pos))
+    grid = torch.empty((G, G, G), dtype=torch.float64, device="cuda")
+    ctx.psd_deposit_uniform(G, grid)
+    assert_mass(grid.sum())
+    assert float(grid.min()) > 0.0
+    mx = float(grid.max())
+    wins, _ = sample_windows(G, n_win, edge, 1000 + cfg_index)
+    wins[0] = (G - 3, G - 5, 0)  # one window across the periodic seam
+    for lo in wins:
+        ora = oracle.deposit_window(pos, 1.0, 1.0, G, lo, (edge,) * 3)
+        got = window_of(grid, lo, edge, G)
+        err = np.abs(got - ora)
+        assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (lo, float(err.max()))
+    s = ctx.psd_get_stats()
+    assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
+    ctx.psd_deposit_uniform(G, grid)
+    assert float((grid - 1.0).abs().max()) < 1e-9
