@@ -9,9 +9,9 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_symbols():
-    src = open(os.path.join(ROOT, "include", "psd.h")).read()
-    return sorted(set(re.findall(r"PSD_API\s+[\w\s\*]+?\b(psd_\w+)\s*\(", src)))
+def header_symbols(header="psd.h", macro="PSD_API"):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    return sorted(set(re.findall(macro + r"\s+[\w\s\*]+?\b(psd_\w+)\s*\(", src)))
 
 
 def test_header_declares_the_north_star_calls():
@@ -30,6 +30,16 @@ def test_library_builds_loads_and_exports_every_symbol():
         assert hasattr(lib, name), f"{name} declared in psd.h but not exported"
     assert sorted(binding.EXPORTS) == syms
     assert binding.version().startswith("libpsd sm_100a")
+
+
+def test_peaks_library_builds_loads_and_exports_every_symbol():
+    from paper_1612_09491_b200 import _build, peaks
+    lib = ctypes.CDLL(_build.build(target=_build.PEAKS_LIB))
+    syms = header_symbols("psd_peaks.h", "PSD_PEAKS_API")
+    assert len(syms) == 4
+    for name in syms:
+        assert hasattr(lib, name), f"{name} declared in psd_peaks.h but not exported"
+    assert sorted(peaks.EXPORTS) == syms
 
 
 def test_stats_struct_matches_header_layout():
