@@ -58,8 +58,8 @@ enum {
                                 any displacement field (a self-check needing no oracle).     */
     PSD_OPT_KERNEL = 1,      /* 0 (default): binned tile path when the grid allows it (G % 8 == 0).
                                 1: direct path (one thread per tet, global atomics).           */
-    PSD_OPT_COUNTERS = 2,    /* 1: also count column tasks / face clips / plane clips / cells
-                                written during deposits (slower; for the roofline model).       */
+    PSD_OPT_COUNTERS = 2,    /* 1: also count face jobs / non-empty clips / plane integrals / cell
+                                shares written during deposits (slower; for the work model).    */
     PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 1024) */
     PSD_OPT_CHORD_AXIS = 4   /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
 };
@@ -88,10 +88,10 @@ typedef struct {
     uint64_t hist_tet[64];  /* tets by b = bit_width(n_cells-1)                          */
     uint64_t hist_pair[64]; /* pairs by b of the tet's cells inside that tile            */
     /* PSD_OPT_COUNTERS = 1 only: */
-    int64_t n_column_tasks; /* (tet, column) tasks run                                   */
-    int64_t n_face_clips;   /* tet faces clipped to a column with non-empty result       */
-    int64_t n_plane_clips;  /* chord-plane clips of a face polygon                       */
-    int64_t n_cells_written;/* cell contributions added to accumulators                  */
+    int64_t n_face_jobs;    /* (tet face, column) jobs run                               */
+    int64_t n_face_clips;   /* jobs whose clipped polygon is non-empty and reaches the run */
+    int64_t n_plane_evals;  /* closed-form lattice-plane integrals of a face polygon     */
+    int64_t n_cells_written;/* per-face cell shares added to accumulators                */
     /* device pointer to the per-tile counts of the last binned deposit (n_tiles uint32) */
     const uint32_t* tile_counts_dev;
     /* device time of the phases of the last deposit, ms (0 if not recorded)             */

@@ -40,7 +40,7 @@ class PsdStats(C.Structure):
         ("n_inverted", C.c_int64), ("n_degenerate", C.c_int64), ("n_unwrap_suspect", C.c_int64),
         ("n_nonfinite", C.c_int64),
         ("hist_tet", C.c_uint64 * 64), ("hist_pair", C.c_uint64 * 64),
-        ("n_column_tasks", C.c_int64), ("n_face_clips", C.c_int64), ("n_plane_clips", C.c_int64),
+        ("n_face_jobs", C.c_int64), ("n_face_clips", C.c_int64), ("n_plane_evals", C.c_int64),
         ("n_cells_written", C.c_int64),
         ("tile_counts_dev", C.c_void_p),
         ("ms_census", C.c_float), ("ms_scan", C.c_float), ("ms_scatter", C.c_float),

@@ -477,9 +477,9 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
         s.n_inverted = (int64_t)ctx->pinned[ST_INVERTED];
         s.n_degenerate = (int64_t)ctx->pinned[ST_DEGENERATE];
         s.n_unwrap_suspect = (int64_t)ctx->pinned[ST_UNWRAP];
-        s.n_column_tasks = (int64_t)ctx->pinned[ST_TASKS];
+        s.n_face_jobs = (int64_t)ctx->pinned[ST_TASKS];
         s.n_face_clips = (int64_t)ctx->pinned[ST_FACE_CLIPS];
-        s.n_plane_clips = (int64_t)ctx->pinned[ST_PLANE_CLIPS];
+        s.n_plane_evals = (int64_t)ctx->pinned[ST_PLANE_CLIPS];
         s.n_cells_written = (int64_t)ctx->pinned[ST_CELLS];
         for (int i = 0; i < 64; ++i) {
             s.hist_tet[i] = ctx->pinned[ST_COUNT + i];

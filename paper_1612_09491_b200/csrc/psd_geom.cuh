@@ -6,18 +6,20 @@
 //   PAPER.md:155-161 exact tet-cube intersection by axis-aligned plane clipping
 //
 // How (differs from the paper's K80 design):
-// the tet is kept as a boundary polytope (its 4 oriented faces).  For one COLUMN of cells
-// (a unit square in two axes, running along the third, "chord" axis u) each face is clipped
-// by the 4 axis-aligned planes of the column (Sutherland-Hodgman, in place), then for every
-// lattice plane u = a crossing the clipped face polygon Q the polygon is clipped once more
-// by u >= a and the prism between it and the plane is integrated by FAN DECOMPOSITION:
-//     R_F(a) = signed integral over Q n {u>=a} of (u - a) dv dw.
-// By the divergence theorem (flux of (u-a,0,0)) the sum over the 4 faces is
+// the tet is kept as a boundary polytope (its 4 oriented faces).  The unit of work is a
+// FACE JOB: one face triangle against one COLUMN of cells (a unit square in two axes, running
+// along the third, "chord" axis u).  The triangle is clipped by the 4 axis-aligned walls of the
+// column (Sutherland-Hodgman, in place) giving a convex polygon Q, on which u is linear.  With
+//     R_F(a) = signed integral over Q n {u >= a} of (u - a) dv dw
+// the divergence theorem (flux of (u-a,0,0)) gives, summed over the 4 faces,
 //     R(a) = vol(T n column n {u >= a}),
-// the cell [a,a+1] receives R(a) - R(a+1): the cell's own faces never need a cap polygon
-// (column walls have zero u-flux and the cap u = a has u-a = 0).  All interpolation is
-// between points on opposite sides of a plane (convex combinations), coordinates are local
-// to the tile/column, arithmetic is fp64.
+// so the cell [a,a+1] receives R(a) - R(a+1): the cell's own faces never need a cap polygon
+// (column walls have zero u-flux and the cap u = a has u-a = 0), and every face adds its own
+// share to the cell independently of the other faces.  R_F(a) is evaluated in CLOSED FORM per
+// fan triangle of Q (the integral of (u-a)_+ over a triangle is a cubic in a between its sorted
+// vertex heights), so a lattice plane costs a few flops, not another clip.  All interpolation
+// is between points on opposite sides of a plane (convex combinations), every ratio used is in
+// [0,1], coordinates are local to the tile/column, arithmetic is fp64.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -175,6 +177,16 @@ __device__ __forceinline__ void load_tet_vertices(const Particles& p, int64_t ce
         for (int x = 0; x < 3; ++x) P[v][x] = unwrap1(P[v][x], P[0][x], p.L);
 }
 
+// 1/x to about 1 ulp for a normal, non-zero x, without the IEEE division's special-case path:
+// hardware seed (MUFU.RCP64H) and two Newton steps.  The clip ratios do not need correct rounding.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
+}
+
 // ------------------------------------------------------------------ polygon buffer
 // One lane's polygon: POLY_CAP vertices x (u,v,w), element stride S doubles
 // (S = 32: warp-interleaved shared memory, bank-conflict free for any index; S = 1: local).
@@ -204,7 +216,7 @@ __device__ __forceinline__ int clip_wall(PolyBuf<S> q, int n) {
             double iu = pin ? pu : cu, iv = pin ? pv : cv, iw = pin ? pw : cw;
             double ou = pin ? cu : pu, ov = pin ? cv : pv, ow = pin ? cw : pw;
             double di = pin ? dp : dc, dout = pin ? dc : dp;
-            double t = di / (di - dout);
+            double t = di * fast_rcp(di - dout);
             double xu = fma(t, ou - iu, iu), xv = fma(t, ov - iv, iv), xw = fma(t, ow - iw, iw);
             if (AX == 1) xv = UP ? 1.0 : 0.0; else xw = UP ? 1.0 : 0.0;
             q.at(m, 0) = xu; q.at(m, 1) = xv; q.at(m, 2) = xw;
@@ -219,129 +231,100 @@ __device__ __forceinline__ int clip_wall(PolyBuf<S> q, int n) {
     return m;
 }
 
-// signed integral over (Q n {u >= a}) of (u - a) dv dw: clip by the chord plane and integrate
-// the prism by a fan from the first emitted vertex, streaming (nothing is stored).
-template <int S>
-__device__ __forceinline__ double chord_integral(PolyBuf<S> q, int n, double a) {
-    double fv = 0, fw = 0, fh = 0, lv = 0, lw = 0, lh = 0, acc = 0;
-    int k = 0;
-    double pu = q.at(n - 1, 0), pv = q.at(n - 1, 1), pw = q.at(n - 1, 2);
-    double dp = pu - a;
-    for (int i = 0; i < n; ++i) {
-        double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
-        double dc = cu - a;
-        bool pin = dp >= 0.0, cin = dc >= 0.0;
-#pragma unroll
-        for (int pass = 0; pass < 2; ++pass) {
-            double ev, ew, eh;
-            bool emit;
-            if (pass == 0) {
-                emit = pin != cin;
-                double iv = pin ? pv : cv, iw = pin ? pw : cw;
-                double ov = pin ? cv : pv, ow = pin ? cw : pw;
-                double di = pin ? dp : dc, dout = pin ? dc : dp;
-                double t = emit ? di / (di - dout) : 0.0;
-                ev = fma(t, ov - iv, iv); ew = fma(t, ow - iw, iw); eh = 0.0;
-            } else {
-                emit = cin;
-                ev = cv; ew = cw; eh = dc;
-            }
-            if (emit) {
-                if (k == 0) { fv = ev; fw = ew; fh = eh; }
-                else if (k > 1) {
-                    double cr = (lv - fv) * (ew - fw) - (lw - fw) * (ev - fv);
-                    acc = fma(cr, fh + lh + eh, acc);
-                }
-                lv = ev; lw = ew; lh = eh;
-                ++k;
-            }
-        }
-        pu = cu; pv = cv; pw = cw; dp = dc;
-    }
-    return acc * (1.0 / 6.0);
+// integral over a triangle of (u - a)_+ dv dw per unit (signed) area, for a lattice plane a
+// strictly between the triangle's lowest and highest vertex; ua, ub, uc are the vertex heights.
+// Sorted u0 <= u1 <= u2:  a >= u1: the part above is the corner triangle at u2, similar with
+// ratios t/(u2-u1), t/(u2-u0), t = u2-a, mean height t/3.  a < u1: whole minus the part below,
+// the corner triangle at u0.  Both ratios are in [0,1]: no cancellation, no blow-up.
+__device__ __forceinline__ double tri_above_unit(double ua, double ub, double uc, double a) {
+    const double lo_ab = fmin(ua, ub), hi_ab = fmax(ua, ub);
+    const double u0 = fmin(lo_ab, uc), u2 = fmax(hi_ab, uc);
+    const double u1 = fmax(lo_ab, fmin(hi_ab, uc));
+    const double lin = (ua + ub + uc) * (1.0 / 3.0) - a;
+    if (a <= u0) return lin;
+    if (a >= u2) return 0.0;
+    const bool hi = a >= u1;
+    const double t = hi ? u2 - a : a - u0;
+    const double d1 = hi ? u2 - u1 : u1 - u0;
+    const double cub = t * t * t * fast_rcp(fmax(3.0 * d1 * (u2 - u0), 1e-290));
+    return hi ? cub : lin + cub;
 }
 
-struct ColumnCounters {
-    unsigned int tasks, face_clips, plane_clips, cells;
+struct JobCounters {
+    unsigned int jobs, face_clips, plane_evals, cells;
 };
 
 // faces of tet (0,1,2,3) with outward orientation when det > 0: (1,2,3) (0,3,2) (0,1,3) (0,2,1)
-// packed 2 bits per vertex index.
+// packed 2 bits per vertex index, 6 bits per face.
 constexpr unsigned FACE_TABLE = (1u | 2u << 2 | 3u << 4) | (0u | 3u << 2 | 2u << 4) << 6 |
                                 (0u | 1u << 2 | 3u << 4) << 12 | (0u | 2u << 2 | 1u << 4) << 18;
 
-// One (tet, column) task.  getv(vertex, comp) returns the tet vertex coordinate with comp 0 = u
-// (chord axis, relative to the first lattice plane of the run), 1 = v, 2 = w (relative to the
-// column's lower corner).  Planes a = 0..na (na <= 8) bound the na cells of the run.
-// emit(c, val) receives the signed overlap volume (cell units) of cell c in [0, na).
-template <int S, bool COUNT, class GetV, class Emit>
-__device__ __forceinline__ void column_task(GetV getv, int na, PolyBuf<S> q, double* rt, Emit emit,
-                                            ColumnCounters* cnt) {
-    for (int a = 0; a <= na; ++a) rt[a * S] = 0.0;
-    double col_min = 1e300, col_max = -1e300;
-    if (COUNT) cnt->tasks++;
-#pragma unroll 1
-    for (int f = 0; f < 4; ++f) {
-        unsigned fv = FACE_TABLE >> (6 * f);
-        double minv = 1e300, maxv = -1e300, minw = 1e300, maxw = -1e300, maxu = -1e300;
+// One FACE JOB.  q holds the face triangle: 3 vertices (u, v, w) with v, w relative to the
+// column's lower corner (the column is the unit square [0,1]^2) and u in the coordinates of the
+// cell run: the run is the cells c_lo..c_hi, cell c spanning u in [c, c+1].
+// emit(c, D) receives the face's signed share D of the overlap volume of cell c (cell units):
+//     D = R_F(c) - R_F(c+1),   R_F(a) = integral over Q n {u >= a} of (u - a) dv dw,
+// Q = triangle n column.  Cells entirely below Q get the signed projected area of Q (the faces
+// of the tet above and below them cancel), cells entirely above Q get nothing.
+template <int S, bool COUNT, class Emit>
+__device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit emit, JobCounters* cnt) {
+    if (COUNT) cnt->jobs++;
+    double minv = 1e300, maxv = -1e300, minw = 1e300, maxw = -1e300;
 #pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            int vi = (fv >> (2 * i)) & 3;
-            double u = getv(vi, 0), v = getv(vi, 1), w = getv(vi, 2);
-            q.at(i, 0) = u; q.at(i, 1) = v; q.at(i, 2) = w;
-            minv = fmin(minv, v); maxv = fmax(maxv, v);
-            minw = fmin(minw, w); maxw = fmax(maxw, w);
-            maxu = fmax(maxu, u);
-        }
-        // no area inside the column, or entirely below the first plane: contributes nothing
-        if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) continue;
-        // a face below the first plane adds nothing to any R(a), but the tet may reach down to it:
-        // the run of cells then starts at cell 0
-        if (maxu <= 0.0) { col_min = fmin(col_min, 0.0); continue; }
-        int n = 3;
-        if (minv < 0.0) n = clip_wall<S, 1, 0>(q, n);
-        if (maxv > 1.0) n = clip_wall<S, 1, 1>(q, n);
-        if (minw < 0.0) n = clip_wall<S, 2, 0>(q, n);
-        if (maxw > 1.0) n = clip_wall<S, 2, 1>(q, n);
-        if (n < 3) continue;
-        if (COUNT) cnt->face_clips++;
-        // signed projected area A and first moment M1 = integral of u, fan from vertex 0
-        double u0 = q.at(0, 0), v0 = q.at(0, 1), w0 = q.at(0, 2);
-        double umin = u0, umax = u0, A2 = 0.0, M6 = 0.0;
-        double lu = q.at(1, 0), lv = q.at(1, 1), lw = q.at(1, 2);
-        umin = fmin(umin, lu); umax = fmax(umax, lu);
-        for (int i = 2; i < n; ++i) {
-            double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
-            double cr = (lv - v0) * (cw - w0) - (lw - w0) * (cv - v0);
-            A2 += cr;
-            M6 = fma(cr, u0 + lu + cu, M6);
-            umin = fmin(umin, cu); umax = fmax(umax, cu);
-            lu = cu; lv = cv; lw = cw;
-        }
-        if (umax <= 0.0) { col_min = fmin(col_min, 0.0); continue; }
-        col_min = fmin(col_min, umin); col_max = fmax(col_max, umax);
-        double A = 0.5 * A2, M1 = M6 * (1.0 / 6.0);
-        for (int a = 0; a <= na; ++a) {
-            double fa = (double)a;
-            if (fa >= umax) break;
-            double R;
-            if (fa <= umin) R = fma(-fa, A, M1);
-            else {
-                R = chord_integral<S>(q, n, fa);
-                if (COUNT) cnt->plane_clips++;
-            }
-            rt[a * S] += R;
-        }
+    for (int i = 0; i < 3; ++i) {
+        double v = q.at(i, 1), w = q.at(i, 2);
+        minv = fmin(minv, v); maxv = fmax(maxv, v);
+        minw = fmin(minw, w); maxw = fmax(maxw, w);
     }
-    if (col_max <= 0.0 || col_min > col_max) return;
-    int c0 = col_min <= 0.0 ? 0 : min((int)col_min, na);
-    int c1 = col_max >= (double)na ? na - 1 : (int)col_max;
-    for (int c = c0; c <= c1; ++c) {
-        double val = rt[c * S] - rt[(c + 1) * S];
-        if (val != 0.0) {
-            emit(c, val);
-            if (COUNT) cnt->cells++;
+    if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) return;
+    int n = 3;
+    if (minv < 0.0) n = clip_wall<S, 1, 0>(q, n);
+    if (maxv > 1.0) n = clip_wall<S, 1, 1>(q, n);
+    if (minw < 0.0) n = clip_wall<S, 2, 0>(q, n);
+    if (maxw > 1.0) n = clip_wall<S, 2, 1>(q, n);
+    if (n < 3) return;
+    // signed projected area A and first moment M1 = integral of u over Q, fan from vertex 0
+    const double u0 = q.at(0, 0), v0 = q.at(0, 1), w0 = q.at(0, 2);
+    double lu = q.at(1, 0), lv = q.at(1, 1), lw = q.at(1, 2);
+    double umin = fmin(u0, lu), umax = fmax(u0, lu), A2 = 0.0, M6 = 0.0;
+    for (int i = 2; i < n; ++i) {
+        double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
+        double cr = (lv - v0) * (cw - w0) - (lw - w0) * (cv - v0);
+        A2 += cr;
+        M6 = fma(cr, u0 + lu + cu, M6);
+        umin = fmin(umin, cu); umax = fmax(umax, cu);
+        lu = cu; lv = cv; lw = cw;
+    }
+    if (umax <= (double)c_lo) return;  // entirely below the run: no share in any of its cells
+    if (COUNT) cnt->face_clips++;
+    const double A = 0.5 * A2, M1 = M6 * (1.0 / 6.0);
+    const int top = umax >= (double)(c_hi + 1) ? c_hi : __double2int_ru(umax) - 1;
+    double Rp = 0.0;
+    for (int a = c_lo; a <= top + 1; ++a) {
+        const double fa = (double)a;
+        double R;
+        if (fa <= umin) R = fma(-fa, A, M1);
+        else if (fa >= umax) R = 0.0;
+        else {
+            // closed form per fan triangle
+            double pu = q.at(1, 0), pv = q.at(1, 1), pw = q.at(1, 2), acc = 0.0;
+            for (int i = 2; i < n; ++i) {
+                double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
+                double cr = (pv - v0) * (cw - w0) - (pw - w0) * (cv - v0);
+                acc = fma(cr, tri_above_unit(u0, pu, cu, fa), acc);
+                pu = cu; pv = cv; pw = cw;
+            }
+            R = 0.5 * acc;
+            if (COUNT) cnt->plane_evals++;
         }
+        if (a > c_lo) {
+            const double D = fa <= umin ? A : Rp - R;
+            if (D != 0.0) {
+                emit(a - 1, D);
+                if (COUNT) cnt->cells++;
+            }
+        }
+        Rp = R;
     }
 }
 

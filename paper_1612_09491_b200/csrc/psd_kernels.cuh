@@ -317,8 +317,9 @@ struct DepositArgs {
 
 constexpr int DEP_WARPS = 4;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
-// per-warp scratch in doubles: tet slots [13][32] + polygon [24][32] + chord planes [9][32]
-constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP + 9) * 32;
+// per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
+// [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32)
+constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP) * 32 + 32 + 16;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
 
 __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile, int& level,
@@ -341,16 +342,24 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
     }
 }
 
+// One CTA per work item (a chunk of one tile's pair list), an 8^3 fp64 accumulator in shared
+// memory.  Each warp takes 32 pairs at a time:
+//   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
+//            into the warp's slots; per face the rectangle of columns its projection meets.
+//   stage B  the face jobs (slot, face, column) of the 32 slots are numbered by a warp prefix
+//            sum of the rectangle sizes; lane = job, 32 jobs at a time, every lane busy.
+//   stage C  face_job: wall clip, closed-form plane integrals, shares added to the tile (a4-a6).
+// The tile is flushed to global memory with fp64 reductions at the end (a6).
 template <bool COUNT>
 __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;  // [13][32]
-    double* wpoly = wtet + 13 * 32;                          // [24][32]
-    double* wrt = wpoly + 3 * POLY_CAP * 32;                 // [9][32]
+    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
+    double* wpoly = wtet + 13 * 32;                                                    // [24][32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * POLY_CAP * 32);  // [32]
+    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 32);                 // [32]
     PolyBuf<32> poly{wpoly + lane};
-    double* rt = wrt + lane;
 
     const Item item = A.items[blockIdx.x];
     int level, org[3];
@@ -363,7 +372,7 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
     for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
     __syncthreads();
 
-    ColumnCounters cnt = {0, 0, 0, 0};
+    JobCounters cnt = {0, 0, 0, 0};
 
     for (unsigned int base = warp * 32; base < item.count; base += DEP_WARPS * 32) {
         // ---- a1: each lane builds one tet of the batch
@@ -386,34 +395,35 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
         int my_images = have ? nimg[0] * nimg[1] * nimg[2] : 0;
         const int max_images = __reduce_max_sync(0xffffffffu, my_images);
         for (int img = 0; img < max_images; ++img) {
-            // ---- slot setup: tile-local vertices, weight, column range
-            int info = 0, ncol = 0;
+            // ---- stage A: slot = lane.  Tile-local vertices, weight, face rectangles.
+            int njobs = 0;
             __syncwarp();
             if (img < my_images) {
                 int m[3] = {mlo[0] + img % nimg[0], mlo[1] + (img / nimg[0]) % nimg[1],
                             mlo[2] + img / (nimg[0] * nimg[1])};
                 int lo[3], hi[3];
+                double gl[4][3];
 #pragma unroll
                 for (int x = 0; x < 3; ++x) {
                     int o = org[x] + m[x] * Gl;
                     lo[x] = max(t.lo[x] - o, 0);
                     hi[x] = min(t.hi[x] - o, TILE - 1);
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) wtet[(3 * v + x) * 32 + lane] = t.g[v][x] - (double)o;
+                    for (int v = 0; v < 4; ++v) {
+                        gl[v][x] = t.g[v][x] - (double)o;
+                        wtet[(3 * v + x) * 32 + lane] = gl[v][x];
+                    }
                 }
-                double w;
-                if (A.weight_mode == 0) w = det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0;
-                else w = 1.0;
-                wtet[12 * 32 + lane] = w;
+                wtet[12 * 32 + lane] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
                 int ax = A.chord_axis;
                 if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
                     int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
                     ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
                 }
-                int av = (ax + 1) % 3, aw = (ax + 2) % 3;
-                ncol = (hi[av] - lo[av] + 1) * (hi[aw] - lo[aw] + 1);
+                const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
+                unsigned long long rect = 0ull;
+                unsigned int cum = 0u;
                 if (det == 0.0) {  // degenerate: whole mass to the centroid cell (Q6)
-                    ncol = 0;
                     if (A.weight_mode == 0) {
                         int c[3];
                         bool in = true;
@@ -425,54 +435,92 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                         }
                         if (in) atomicAdd(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], A.mass_per_tet);
                     }
+                } else {
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
+                        double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300, mxu = -1e300;
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            if (v == f) continue;
+                            // av, aw, ax are runtime: select instead of indexing
+                            double cu = ax == 0 ? gl[v][0] : (ax == 1 ? gl[v][1] : gl[v][2]);
+                            double cv = av == 0 ? gl[v][0] : (av == 1 ? gl[v][1] : gl[v][2]);
+                            double cw = aw == 0 ? gl[v][0] : (aw == 1 ? gl[v][1] : gl[v][2]);
+                            mnv = fmin(mnv, cv); mxv = fmax(mxv, cv);
+                            mnw = fmin(mnw, cw); mxw = fmax(mxw, cw);
+                            mxu = fmax(mxu, cu);
+                        }
+                        const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
+                        const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
+                        const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
+                        const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
+                        const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                        // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
+                        const int v0 = max(__double2int_rd(mnv), lov), v1 = min(__double2int_ru(mxv) - 1, hiv);
+                        const int w0 = max(__double2int_rd(mnw), low), w1 = min(__double2int_ru(mxw) - 1, hiw);
+                        int c = 0;
+                        if (v1 >= v0 && w1 >= w0 && mxu > (double)lou) {
+                            c = (v1 - v0 + 1) * (w1 - w0 + 1);
+                            rect |= (unsigned long long)(v0 | (v1 - v0) << 3 | w0 << 6 | (w1 - w0) << 9) << (16 * f);
+                        }
+                        njobs += c;
+                        if (f < 3) cum |= (unsigned int)njobs << (8 + 8 * f);
+                    }
                 }
-                info = lo[ax] | (hi[ax] << 3) | lo[av] << 6 | (hi[av] - lo[av]) << 9 | lo[aw] << 12 |
-                       (hi[aw] - lo[aw]) << 15 | ax << 18;
+                const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
+                wrect[lane] = rect;
+                wword[lane] = cum | (unsigned int)(ax | lou << 2 | hiu << 5);
             }
-            // ---- exclusive prefix of column counts over the 32 slots
-            int pre = ncol;
+            // ---- stage B: exclusive prefix of the job counts over the 32 slots
+            int pre = njobs;
             for (int o = 1; o < 32; o <<= 1) {
                 int y = __shfl_up_sync(0xffffffffu, pre, o);
                 if (lane >= o) pre += y;
             }
             const int total = __shfl_sync(0xffffffffu, pre, 31);
-            pre -= ncol;
+            pre -= njobs;
             __syncwarp();
-            // ---- a4-a6: columns of all 32 tets spread evenly over the lanes
-            for (int cb = 0; cb < total; cb += 32) {
-                const int cand = cb + lane;
-                int slot = 0;  // largest slot with pre[slot] <= cand
+            for (int jb = 0; jb < total; jb += 32) {
+                const int job = jb + lane;
+                int slot = 0;  // largest slot with pre[slot] <= job
 #pragma unroll
                 for (int step = 16; step; step >>= 1) {
                     int probe = __shfl_sync(0xffffffffu, pre, slot + step);
-                    if (probe <= cand) slot += step;
+                    if (probe <= job) slot += step;
                 }
-                const int sinfo = __shfl_sync(0xffffffffu, info, slot);
                 const int spre = __shfl_sync(0xffffffffu, pre, slot);
-                if (cand < total) {
-                    const int a0 = sinfo & 7, a1 = (sinfo >> 3) & 7;
-                    const int v0 = (sinfo >> 6) & 7, w0 = (sinfo >> 12) & 7;
-                    const int nw = ((sinfo >> 15) & 7) + 1;
-                    const int ax = (sinfo >> 18) & 3;
+                if (job < total) {
+                    // ---- decode (slot, face, column)
+                    const unsigned int word = wword[slot];
+                    int local = job - spre;
+                    const int c1 = (word >> 8) & 255, c2 = (word >> 16) & 255, c3 = word >> 24;
+                    const int f = (local >= c1) + (local >= c2) + (local >= c3);
+                    local -= f == 0 ? 0 : (f == 1 ? c1 : (f == 2 ? c2 : c3));
+                    const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
+                    const int nw = ((r16 >> 9) & 7) + 1;
+                    const int cv = (r16 & 7) + local / nw, cw = ((r16 >> 6) & 7) + local % nw;
+                    const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-                    const int local = cand - spre;
-                    const int cv = v0 + local / nw, cw = w0 + local % nw;
+                    // ---- stage C: the face triangle, column-local, into the lane's polygon buffer
                     const double* ts = wtet + slot;
-                    const double ou = (double)a0, ov = (double)cv, ow = (double)cw;
-                    auto getv = [&](int vi, int comp) -> double {
-                        int axis = comp == 0 ? ax : (comp == 1 ? av : aw);
-                        double off = comp == 0 ? ou : (comp == 1 ? ov : ow);
-                        return ts[(3 * vi + axis) * 32] - off;
-                    };
+                    const unsigned int fv = FACE_TABLE >> (6 * f);
+                    const double ov = (double)cv, ow = (double)cw;
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) {
+                        const int vi = (fv >> (2 * i)) & 3;
+                        poly.at(i, 0) = ts[(3 * vi + ax) * 32];
+                        poly.at(i, 1) = ts[(3 * vi + av) * 32] - ov;
+                        poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
+                    }
                     const double w = ts[12 * 32];
                     // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
                     const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
                     const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
                     const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
-                    double* col = acc + a0 * su + cv * sv + cw * sw;
-                    column_task<32, COUNT>(getv, a1 - a0 + 1, poly, rt,
-                                           [&](int c, double val) { atomicAdd(col + c * su, w * val); },
-                                           &cnt);
+                    double* col = acc + cv * sv + cw * sw;
+                    face_job<32, COUNT>(poly, c_lo, c_hi,
+                                        [&](int c, double D) { atomicAdd(col + c * su, w * D); }, &cnt);
                 }
             }
         }
@@ -487,8 +535,8 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
         }
     }
     if (COUNT) {
-        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.tasks), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
-        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_clips), d = __reduce_add_sync(0xffffffffu, cnt.cells);
+        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.jobs), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
+        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_evals), d = __reduce_add_sync(0xffffffffu, cnt.cells);
         if (lane == 0) {
             atomicAdd(&A.stats[ST_TASKS], (unsigned long long)a);
             atomicAdd(&A.stats[ST_FACE_CLIPS], (unsigned long long)b);
@@ -499,13 +547,14 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
 }
 
 // ---------------------------------------------------------------- direct path (any G)
-// One thread per tet, polygon in local memory, global fp64 atomics with periodic wrap.
-// The plain first path: kept as PSD_OPT_KERNEL = 1 and for grids the tiling does not divide.
+// One thread per tet, all its face jobs in sequence, polygon in local memory, global fp64
+// atomics with periodic wrap.  The plain path: PSD_OPT_KERNEL = 1, and grids the tiling does
+// not divide.
 template <bool COUNT>
 __global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
     const int64_t ntet = (int64_t)6 * A.part.N * A.part.N * A.part.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    ColumnCounters cnt = {0, 0, 0, 0};
+    JobCounters cnt = {0, 0, 0, 0};
     if (id < ntet) {
         const Space& s = A.space;
         const int G = s.G;
@@ -524,7 +573,7 @@ __global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
             }
         } else {
             const double w = A.weight_mode == 0 ? 6.0 * A.mass_per_tet / det : 1.0;
-            double polymem[3 * POLY_CAP], rtmem[9];
+            double polymem[3 * POLY_CAP];
             PolyBuf<1> poly{polymem};
             int ax = A.chord_axis;
             if (ax < 0) {
@@ -532,27 +581,44 @@ __global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
                 ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
             }
             const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
-            for (int cv = t.lo[av]; cv <= t.hi[av]; ++cv)
-                for (int cw = t.lo[aw]; cw <= t.hi[aw]; ++cw)
-                    for (int u0 = t.lo[ax]; u0 <= t.hi[ax]; u0 += TILE) {
-                        int na = min(TILE, t.hi[ax] - u0 + 1);
-                        auto getv = [&](int vi, int comp) -> double {
-                            int axis = comp == 0 ? ax : (comp == 1 ? av : aw);
-                            double off = comp == 0 ? (double)u0 : (comp == 1 ? (double)cv : (double)cw);
-                            // dynamic index into t.g: local memory, fine for this path
-                            return t.g[vi][axis] - off;
-                        };
-                        column_task<1, COUNT>(getv, na, poly, rtmem, [&](int c, double val) {
+            // coordinates local to the tet's first cell (dynamic indexing: local memory, fine here)
+            double gl[4][3];
+            for (int v = 0; v < 4; ++v)
+                for (int x = 0; x < 3; ++x) gl[v][x] = t.g[v][x] - (double)t.lo[x];
+            const int nu = t.hi[ax] - t.lo[ax], nv = t.hi[av] - t.lo[av], nw = t.hi[aw] - t.lo[aw];
+#pragma unroll 1
+            for (int f = 0; f < 4; ++f) {
+                const unsigned int fv = FACE_TABLE >> (6 * f);
+                double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300;
+                for (int i = 0; i < 3; ++i) {
+                    const int vi = (fv >> (2 * i)) & 3;
+                    mnv = fmin(mnv, gl[vi][av]); mxv = fmax(mxv, gl[vi][av]);
+                    mnw = fmin(mnw, gl[vi][aw]); mxw = fmax(mxw, gl[vi][aw]);
+                }
+                const int v0 = max(__double2int_rd(mnv), 0), v1 = min(__double2int_ru(mxv) - 1, nv);
+                const int w0 = max(__double2int_rd(mnw), 0), w1 = min(__double2int_ru(mxw) - 1, nw);
+                for (int cv = v0; cv <= v1; ++cv)
+                    for (int cw = w0; cw <= w1; ++cw) {
+                        for (int i = 0; i < 3; ++i) {
+                            const int vi = (fv >> (2 * i)) & 3;
+                            poly.at(i, 0) = gl[vi][ax];
+                            poly.at(i, 1) = gl[vi][av] - (double)cv;
+                            poly.at(i, 2) = gl[vi][aw] - (double)cw;
+                        }
+                        face_job<1, COUNT>(poly, 0, nu, [&](int c, double D) {
                             int cc[3];
-                            cc[ax] = wrap_mod(u0 + c, G); cc[av] = wrap_mod(cv, G); cc[aw] = wrap_mod(cw, G);
-                            atomicAdd(&s.out[((long long)cc[0] * G + cc[1]) * G + cc[2]], w * val);
+                            cc[ax] = wrap_mod(t.lo[ax] + c, G);
+                            cc[av] = wrap_mod(t.lo[av] + cv, G);
+                            cc[aw] = wrap_mod(t.lo[aw] + cw, G);
+                            atomicAdd(&s.out[((long long)cc[0] * G + cc[1]) * G + cc[2]], w * D);
                         }, &cnt);
                     }
+            }
         }
     }
     if (COUNT) {
-        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.tasks), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
-        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_clips), d = __reduce_add_sync(0xffffffffu, cnt.cells);
+        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.jobs), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
+        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_evals), d = __reduce_add_sync(0xffffffffu, cnt.cells);
         if ((threadIdx.x & 31) == 0) {
             atomicAdd(&A.stats[ST_TASKS], (unsigned long long)a);
             atomicAdd(&A.stats[ST_FACE_CLIPS], (unsigned long long)b);

@@ -53,7 +53,7 @@ def test_sample_fraction_bounds_the_cpu_work():
     for cfg in psd_inputs.CONFIGS:
         f = bench.sample_fraction(cfg)
         assert 0.0 < f <= 1.0
-        assert f * 6 * cfg["N"] ** 3 <= 1.5e6 + 1 or cfg["N"] <= 64
+        assert f * 6 * cfg["N"] ** 3 <= 15e6 + 1
 
 
 def test_reference_arm_prints_one_json_line_with_the_contract_keys():
