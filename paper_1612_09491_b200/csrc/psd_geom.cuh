@@ -196,58 +196,129 @@ struct PolyBuf {
     __device__ __forceinline__ double& at(int i, int c) { return p[(3 * i + c) * S]; }
 };
 
-// In-place Sutherland-Hodgman of a convex polygon against one wall of the column:
-// AX = 1 (v) or 2 (w); UP = 0 keeps coord >= 0, UP = 1 keeps coord <= 1.  Vertices exactly on
-// the plane are inside; a crossing is computed only between strictly opposite sides, always
-// from the inside endpoint, so the two faces sharing a tet edge get the identical point.
-template <int S, int AX, int UP>
-__device__ __forceinline__ int clip_wall(PolyBuf<S> q, int n) {
-    if (n == 0) return 0;
-    int m = 0;
-    double pu = q.at(n - 1, 0), pv = q.at(n - 1, 1), pw = q.at(n - 1, 2);
-    double dp = UP ? 1.0 - (AX == 1 ? pv : pw) : (AX == 1 ? pv : pw);
-    double nu = q.at(0, 0), nv = q.at(0, 1), nw = q.at(0, 2);
-    for (int i = 0; i < n; ++i) {
-        double cu = nu, cv = nv, cw = nw;
-        if (i + 1 < n) { nu = q.at(i + 1, 0); nv = q.at(i + 1, 1); nw = q.at(i + 1, 2); }
-        double dc = UP ? 1.0 - (AX == 1 ? cv : cw) : (AX == 1 ? cv : cw);
-        bool pin = dp >= 0.0, cin = dc >= 0.0;
-        if (pin != cin) {
-            double iu = pin ? pu : cu, iv = pin ? pv : cv, iw = pin ? pw : cw;
-            double ou = pin ? cu : pu, ov = pin ? cv : pv, ow = pin ? cw : pw;
-            double di = pin ? dp : dc, dout = pin ? dc : dp;
-            double t = di * fast_rcp(di - dout);
-            double xu = fma(t, ou - iu, iu), xv = fma(t, ov - iv, iv), xw = fma(t, ow - iw, iw);
-            if (AX == 1) xv = UP ? 1.0 : 0.0; else xw = UP ? 1.0 : 0.0;
-            q.at(m, 0) = xu; q.at(m, 1) = xv; q.at(m, 2) = xw;
-            ++m;
-        }
-        if (cin) {
-            q.at(m, 0) = cu; q.at(m, 1) = cv; q.at(m, 2) = cw;
-            ++m;
-        }
-        pu = cu; pv = cv; pw = cw; dp = dc;
-    }
-    return m;
+
+// A convex polygon as a CYCLIC ORDER over storage slots: nibble i of `order` is the slot (0..6)
+// holding vertex i; vertices never move, a clip only writes its two new points and re-packs the
+// order word.  Slots 0..2 hold the face triangle; each clip allocates at most one fresh slot
+// (`fresh`), so 3 + 4 walls = 7 slots suffice (POLY_CAP = 8).
+struct PolyRef {
+    unsigned order;
+    int n;
+    int fresh;
+};
+
+__device__ __forceinline__ int slot_of(unsigned order, int i) { return (order >> (4 * i)) & 7; }
+__device__ __forceinline__ unsigned nib_mask(int n) { return n >= 8 ? 0xffffffffu : ((1u << (4 * n)) - 1u); }
+
+// The two edges where a convex polygon with inside-bits `mask` (bit i: vertex i inside, neither
+// empty nor full) crosses a line: i_out = first outside vertex after an inside one, i_in = first
+// inside vertex after an outside one (cyclic).
+__device__ __forceinline__ void crossing_edges(unsigned mask, int n, int& i_out, int& i_in) {
+    const unsigned full = (1u << n) - 1u;
+    const unsigned prev = ((mask << 1) | (mask >> (n - 1))) & full;  // bit i = inside(i-1)
+    i_out = __ffs(prev & ~mask) - 1;
+    i_in = __ffs(~prev & mask & full) - 1;
 }
 
-// integral over a triangle of (u - a)_+ dv dw per unit (signed) area, for a lattice plane a
-// strictly between the triangle's lowest and highest vertex; ua, ub, uc are the vertex heights.
-// Sorted u0 <= u1 <= u2:  a >= u1: the part above is the corner triangle at u2, similar with
-// ratios t/(u2-u1), t/(u2-u0), t = u2-a, mean height t/3.  a < u1: whole minus the part below,
-// the corner triangle at u0.  Both ratios are in [0,1]: no cancellation, no blow-up.
-__device__ __forceinline__ double tri_above_unit(double ua, double ub, double uc, double a) {
-    const double lo_ab = fmin(ua, ub), hi_ab = fmax(ua, ub);
-    const double u0 = fmin(lo_ab, uc), u2 = fmax(hi_ab, uc);
-    const double u1 = fmax(lo_ab, fmin(hi_ab, uc));
-    const double lin = (ua + ub + uc) * (1.0 / 3.0) - a;
-    if (a <= u0) return lin;
-    if (a >= u2) return 0.0;
-    const bool hi = a >= u1;
-    const double t = hi ? u2 - a : a - u0;
-    const double d1 = hi ? u2 - u1 : u1 - u0;
-    const double cub = t * t * t * fast_rcp(fmax(3.0 * d1 * (u2 - u0), 1e-290));
-    return hi ? cub : lin + cub;
+// Clip the polygon against one wall of the column: wall 0: v >= 0, 1: v <= 1, 2: w >= 0,
+// 3: w <= 1 (a runtime value, so lanes clipping different walls run the same instructions).
+// Vertices exactly on the wall are inside; a convex polygon crosses the wall on exactly two edges,
+// each crossing is interpolated from its inside endpoint (ratio in [0,1]) and put exactly on the wall.
+template <int S>
+__device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
+    const int ax = 1 + (wall >> 1);
+    const bool up = wall & 1;
+    unsigned mask = 0;
+    for (int i = 0; i < r.n; ++i) {
+        const double x = q.at(slot_of(r.order, i), ax);
+        mask |= (unsigned)((up ? 1.0 - x : x) >= 0.0) << i;
+    }
+    const unsigned full = (1u << r.n) - 1u;
+    if (mask == full) return;
+    if (mask == 0) { r.n = 0; return; }
+    int i_out, i_in;
+    crossing_edges(mask, r.n, i_out, i_in);
+    const int sa = slot_of(r.order, i_out ? i_out - 1 : r.n - 1), sb = slot_of(r.order, i_out);
+    const int sc = slot_of(r.order, i_in ? i_in - 1 : r.n - 1), se = slot_of(r.order, i_in);
+    const double wallpos = up ? 1.0 : 0.0;
+    double xo[3], xi[3];
+    {   // leaving crossing: inside a -> outside b
+        const double a0 = q.at(sa, 0), a1 = q.at(sa, 1), a2 = q.at(sa, 2);
+        const double b0 = q.at(sb, 0), b1 = q.at(sb, 1), b2 = q.at(sb, 2);
+        const double ca = ax == 1 ? a1 : a2, cb = ax == 1 ? b1 : b2;
+        const double da = up ? 1.0 - ca : ca, db = up ? 1.0 - cb : cb;
+        const double t = da * fast_rcp(da - db);
+        xo[0] = fma(t, b0 - a0, a0); xo[1] = fma(t, b1 - a1, a1); xo[2] = fma(t, b2 - a2, a2);
+    }
+    {   // entering crossing: inside e -> outside c
+        const double e0 = q.at(se, 0), e1 = q.at(se, 1), e2 = q.at(se, 2);
+        const double c0 = q.at(sc, 0), c1 = q.at(sc, 1), c2 = q.at(sc, 2);
+        const double ce = ax == 1 ? e1 : e2, cc = ax == 1 ? c1 : c2;
+        const double de = up ? 1.0 - ce : ce, dc = up ? 1.0 - cc : cc;
+        const double t = de * fast_rcp(de - dc);
+        xi[0] = fma(t, c0 - e0, e0); xi[1] = fma(t, c1 - e1, e1); xi[2] = fma(t, c2 - e2, e2);
+    }
+    if (ax == 1) { xo[1] = wallpos; xi[1] = wallpos; } else { xo[2] = wallpos; xi[2] = wallpos; }
+    // new points go to the slots of the first and last removed vertex (already read); if only one
+    // vertex was removed the second point takes a fresh slot
+    const int s_out = sb;
+    int s_in = sc;
+    if (sc == sb) s_in = r.fresh++;
+    q.at(s_out, 0) = xo[0]; q.at(s_out, 1) = xo[1]; q.at(s_out, 2) = xo[2];
+    q.at(s_in, 0) = xi[0]; q.at(s_in, 1) = xi[1]; q.at(s_in, 2) = xi[2];
+    // order: X_in, the inside run (starting at i_in), X_out
+    const int m = __popc(mask);
+    const unsigned rot = i_in ? ((r.order >> (4 * i_in)) | (r.order << (4 * (r.n - i_in)))) : r.order;
+    r.order = (unsigned)s_in | ((rot & nib_mask(m)) << 4) | ((unsigned)s_out << (4 * (m + 1)));
+    r.n = m + 2;
+}
+
+// R(a) = integral over Q n {u >= a} of (u - a) dv dw for a plane strictly between the polygon's
+// lowest and highest vertex: Q is cut by the line u = a (two crossings X_in, X_out with u - a = 0,
+// not stored), and the kept part [X_in, inside run, X_out] is fanned from X_in.  Every fan triangle
+// lies inside Q and every height is >= 0: a sum of same-signed terms, no cancellation.
+// Returns 6 R (signed like the polygon's orientation).
+template <int S>
+__device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, int n, double a) {
+    unsigned mask = 0;
+    for (int i = 0; i < n; ++i) mask |= (unsigned)(q.at(slot_of(order, i), 0) >= a) << i;
+    const unsigned full = (1u << n) - 1u;
+    if (mask == 0 || mask == full) return 0.0;  // not a cutting plane (caller excludes this)
+    int i_out, i_in;
+    crossing_edges(mask, n, i_out, i_in);
+    const int sa = slot_of(order, i_out ? i_out - 1 : n - 1), sb = slot_of(order, i_out);
+    const int sc = slot_of(order, i_in ? i_in - 1 : n - 1);
+    double x0v, x0w, xov, xow;
+    {
+        const double ha = q.at(sa, 0) - a, hb = q.at(sb, 0) - a;
+        const double t = ha * fast_rcp(ha - hb);
+        const double av = q.at(sa, 1), aw = q.at(sa, 2);
+        xov = fma(t, q.at(sb, 1) - av, av); xow = fma(t, q.at(sb, 2) - aw, aw);
+    }
+    const unsigned rot = i_in ? ((order >> (4 * i_in)) | (order << (4 * (n - i_in)))) : order;
+    const int m = __popc(mask);
+    double pv, pw, ph;  // first inside vertex, relative to X_in
+    {
+        const int se = rot & 7;
+        const double he = q.at(se, 0) - a, hc = q.at(sc, 0) - a;
+        const double t = he * fast_rcp(he - hc);
+        const double ev = q.at(se, 1), ew = q.at(se, 2);
+        x0v = fma(t, q.at(sc, 1) - ev, ev); x0w = fma(t, q.at(sc, 2) - ew, ew);
+        pv = ev - x0v; pw = ew - x0w; ph = he;
+    }
+    double sum = 0.0;
+    for (int j = 1; j <= m; ++j) {
+        double cv, cw, ch;
+        if (j < m) {
+            const int s = (rot >> (4 * j)) & 7;
+            cv = q.at(s, 1) - x0v; cw = q.at(s, 2) - x0w; ch = q.at(s, 0) - a;
+        } else {
+            cv = xov - x0v; cw = xow - x0w; ch = 0.0;
+        }
+        sum = fma(pv * cw - pw * cv, ph + ch, sum);
+        pv = cv; pw = cw; ph = ch;
+    }
+    return sum;
 }
 
 struct JobCounters {
@@ -259,16 +330,20 @@ struct JobCounters {
 constexpr unsigned FACE_TABLE = (1u | 2u << 2 | 3u << 4) | (0u | 3u << 2 | 2u << 4) << 6 |
                                 (0u | 1u << 2 | 3u << 4) << 12 | (0u | 2u << 2 | 1u << 4) << 18;
 
-// One FACE JOB.  q holds the face triangle: 3 vertices (u, v, w) with v, w relative to the
-// column's lower corner (the column is the unit square [0,1]^2) and u in the coordinates of the
-// cell run: the run is the cells c_lo..c_hi, cell c spanning u in [c, c+1].
-// emit(c, D) receives the face's signed share D of the overlap volume of cell c (cell units):
-//     D = R_F(c) - R_F(c+1),   R_F(a) = integral over Q n {u >= a} of (u - a) dv dw,
-// Q = triangle n column.  Cells entirely below Q get the signed projected area of Q (the faces
-// of the tet above and below them cancel), cells entirely above Q get nothing.
-template <int S, bool COUNT, class Emit>
-__device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit emit, JobCounters* cnt) {
-    if (COUNT) cnt->jobs++;
+// Result of clipping one face triangle to one column (Q = triangle n column).
+struct FaceClip {
+    unsigned order;
+    int n;            // 0: empty
+    double A, M1;     // signed projected area of Q, first moment integral of u over Q
+    double umin, umax;
+};
+
+// q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
+// corner (the column is the unit square [0,1]^2).
+template <int S>
+__device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
+    FaceClip fc;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.umin = fc.umax = 0.0;
     double minv = 1e300, maxv = -1e300, minw = 1e300, maxw = -1e300;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
@@ -276,55 +351,78 @@ __device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit 
         minv = fmin(minv, v); maxv = fmax(maxv, v);
         minw = fmin(minw, w); maxw = fmax(maxw, w);
     }
-    if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) return;
-    int n = 3;
-    if (minv < 0.0) n = clip_wall<S, 1, 0>(q, n);
-    if (maxv > 1.0) n = clip_wall<S, 1, 1>(q, n);
-    if (minw < 0.0) n = clip_wall<S, 2, 0>(q, n);
-    if (maxw > 1.0) n = clip_wall<S, 2, 1>(q, n);
-    if (n < 3) return;
+    if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) return fc;
+    PolyRef r{0x210u, 3, 3};
+    unsigned pending = (unsigned)(minv < 0.0) | (unsigned)(maxv > 1.0) << 1 | (unsigned)(minw < 0.0) << 2 |
+                       (unsigned)(maxw > 1.0) << 3;
+    while (pending && r.n) {
+        const int wall = __ffs(pending) - 1;
+        pending &= pending - 1;
+        clip_wall<S>(q, r, wall);
+    }
+    if (r.n < 3) return fc;
     // signed projected area A and first moment M1 = integral of u over Q, fan from vertex 0
-    const double u0 = q.at(0, 0), v0 = q.at(0, 1), w0 = q.at(0, 2);
-    double lu = q.at(1, 0), lv = q.at(1, 1), lw = q.at(1, 2);
+    const int s0 = slot_of(r.order, 0), s1 = slot_of(r.order, 1);
+    const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
+    double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
     double umin = fmin(u0, lu), umax = fmax(u0, lu), A2 = 0.0, M6 = 0.0;
-    for (int i = 2; i < n; ++i) {
-        double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
-        double cr = (lv - v0) * (cw - w0) - (lw - w0) * (cv - v0);
+    for (int i = 2; i < r.n; ++i) {
+        const int s = slot_of(r.order, i);
+        const double cu = q.at(s, 0), cv = q.at(s, 1) - v0, cw = q.at(s, 2) - w0;
+        const double cr = lv * cw - lw * cv;
         A2 += cr;
         M6 = fma(cr, u0 + lu + cu, M6);
         umin = fmin(umin, cu); umax = fmax(umax, cu);
         lu = cu; lv = cv; lw = cw;
     }
-    if (umax <= (double)c_lo) return;  // entirely below the run: no share in any of its cells
+    fc.order = r.order; fc.n = r.n;
+    fc.A = 0.5 * A2; fc.M1 = M6 * (1.0 / 6.0);
+    fc.umin = umin; fc.umax = umax;
+    return fc;
+}
+
+// Cells and planes of a clipped face over the run of cells c_lo..c_hi (cell c spans u in [c,c+1]).
+// The face's signed share of cell c is D(c) = R(c) - R(c+1), R(a) = integral over Q n {u >= a} of
+// (u - a) dv dw:  R(a) = M1 - a A for a <= umin, 0 for a >= umax, plane_integral6/6 in between.
+//   trivial part   cells c_lo..t_hi:  A if c+1 <= umin, else M1 - c A (the cell holding umin)
+//   cutting planes a_first..a_last (umin < a < umax): +R(a) to cell a (if <= c_hi), -R(a) to
+//                  cell a-1 (if >= c_lo)
+struct FaceRun {
+    int t_hi;             // last cell of the trivial part (< c_lo: none)
+    int a_first, a_last;  // cutting planes (a_last < a_first: none)
+};
+__device__ __forceinline__ FaceRun face_run(const FaceClip& fc, int c_lo, int c_hi) {
+    FaceRun fr;
+    fr.t_hi = c_lo - 1; fr.a_first = 0; fr.a_last = -1;
+    if (fc.n < 3 || fc.umax <= (double)c_lo) return fr;
+    const int fl = fc.umin >= (double)(c_hi + 1) ? c_hi + 1 : __double2int_rd(fc.umin);  // clamp before converting
+    const int ce = fc.umax >= (double)(c_hi + 2) ? c_hi + 2 : __double2int_ru(fc.umax);
+    const int top = min(c_hi, ce - 1);
+    fr.t_hi = min(top, fl);
+    fr.a_first = max(c_lo, fl + 1);
+    fr.a_last = min(c_hi + 1, ce - 1);
+    return fr;
+}
+
+// One FACE JOB in a single thread (the direct path): emit(c, D) receives the signed shares.
+template <int S, bool COUNT, class Emit>
+__device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit emit, JobCounters* cnt) {
+    if (COUNT) cnt->jobs++;
+    const FaceClip fc = face_clip<S>(q);
+    const FaceRun fr = face_run(fc, c_lo, c_hi);
+    if (fc.n < 3 || fc.umax <= (double)c_lo) return;
     if (COUNT) cnt->face_clips++;
-    const double A = 0.5 * A2, M1 = M6 * (1.0 / 6.0);
-    const int top = umax >= (double)(c_hi + 1) ? c_hi : __double2int_ru(umax) - 1;
-    double Rp = 0.0;
-    for (int a = c_lo; a <= top + 1; ++a) {
-        const double fa = (double)a;
-        double R;
-        if (fa <= umin) R = fma(-fa, A, M1);
-        else if (fa >= umax) R = 0.0;
-        else {
-            // closed form per fan triangle
-            double pu = q.at(1, 0), pv = q.at(1, 1), pw = q.at(1, 2), acc = 0.0;
-            for (int i = 2; i < n; ++i) {
-                double cu = q.at(i, 0), cv = q.at(i, 1), cw = q.at(i, 2);
-                double cr = (pv - v0) * (cw - w0) - (pw - w0) * (cv - v0);
-                acc = fma(cr, tri_above_unit(u0, pu, cu, fa), acc);
-                pu = cu; pv = cv; pw = cw;
-            }
-            R = 0.5 * acc;
-            if (COUNT) cnt->plane_evals++;
+    for (int c = c_lo; c <= fr.t_hi; ++c) {
+        const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
+        if (D != 0.0) { emit(c, D); if (COUNT) cnt->cells++; }
+    }
+    for (int a = fr.a_first; a <= fr.a_last; ++a) {
+        const double R = plane_integral6<S>(q, fc.order, fc.n, (double)a) * (1.0 / 6.0);
+        if (COUNT) cnt->plane_evals++;
+        if (R != 0.0) {
+            if (a <= c_hi) { emit(a, R); if (COUNT) cnt->cells++; }
+            if (a - 1 >= c_lo) { emit(a - 1, -R); if (COUNT) cnt->cells++; }
         }
-        if (a > c_lo) {
-            const double D = fa <= umin ? A : Rp - R;
-            if (D != 0.0) {
-                emit(a - 1, D);
-                if (COUNT) cnt->cells++;
-            }
-        }
-        Rp = R;
     }
 }
 

@@ -369,12 +369,18 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
     const double scale = level_scale(A.space, level);
     const int Gl = level_G(A.space, level);
 
+    __shared__ unsigned int sh_next;  // next batch of 32 pairs: warps fetch batches as they finish
     for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
+    if (threadIdx.x == 0) sh_next = 0u;
     __syncthreads();
 
     JobCounters cnt = {0, 0, 0, 0};
 
-    for (unsigned int base = warp * 32; base < item.count; base += DEP_WARPS * 32) {
+    for (;;) {
+        unsigned int base = 0;
+        if (lane == 0) base = atomicAdd(&sh_next, 32u);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= item.count) break;
         // ---- a1: each lane builds one tet of the batch
         const bool have = base + lane < item.count;
         Tet t;
@@ -490,8 +496,12 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                     if (probe <= job) slot += step;
                 }
                 const int spre = __shfl_sync(0xffffffffu, pre, slot);
+                // ---- stage C1: lane = face job.  Wall clip; the polygon stays in the lane's buffer.
+                unsigned int f_order = 0, f_info = 0;
+                int f_afirst = 0, k = 0;
+                double f_w = 0.0;
                 if (job < total) {
-                    // ---- decode (slot, face, column)
+                    // decode (slot, face, column)
                     const unsigned int word = wword[slot];
                     int local = job - spre;
                     const int c1 = (word >> 8) & 255, c2 = (word >> 16) & 255, c3 = word >> 24;
@@ -502,7 +512,7 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                     const int cv = (r16 & 7) + local / nw, cw = ((r16 >> 6) & 7) + local % nw;
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-                    // ---- stage C: the face triangle, column-local, into the lane's polygon buffer
+                    // the face triangle, column-local, into slots 0..2 of the lane's polygon buffer
                     const double* ts = wtet + slot;
                     const unsigned int fv = FACE_TABLE >> (6 * f);
                     const double ov = (double)cv, ow = (double)cw;
@@ -513,15 +523,72 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                         poly.at(i, 1) = ts[(3 * vi + av) * 32] - ov;
                         poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
                     }
-                    const double w = ts[12 * 32];
-                    // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
-                    const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
-                    const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
-                    const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
-                    double* col = acc + cv * sv + cw * sw;
-                    face_job<32, COUNT>(poly, c_lo, c_hi,
-                                        [&](int c, double D) { atomicAdd(col + c * su, w * D); }, &cnt);
+                    f_w = ts[12 * 32];
+                    if (COUNT) cnt.jobs++;
+                    const FaceClip fc = face_clip<32>(poly);
+                    if (fc.n >= 3 && fc.umax > (double)c_lo) {
+                        if (COUNT) cnt.face_clips++;
+                        const FaceRun fr = face_run(fc, c_lo, c_hi);
+                        // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
+                        const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
+                        const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
+                        const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
+                        const int colofs = cv * sv + cw * sw;
+                        // trivial part: cells entirely below Q get its projected area, the cell
+                        // holding umin gets M1 - c A
+                        for (int c = c_lo; c <= fr.t_hi; ++c) {
+                            const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
+                            if (D != 0.0) {
+                                atomicAdd(acc + colofs + c * su, f_w * D);
+                                if (COUNT) cnt.cells++;
+                            }
+                        }
+                        k = max(fr.a_last - fr.a_first + 1, 0);
+                        f_order = fc.order;
+                        f_afirst = fr.a_first;
+                        f_info = (unsigned)colofs | (unsigned)ax << 9 | (unsigned)c_lo << 11 | (unsigned)c_hi << 14 |
+                                 (unsigned)fc.n << 17;
+                    }
                 }
+                // ---- stage C2: the cutting planes (polygon, a) of the 32 jobs, numbered by a warp
+                // prefix sum; lane = plane.  The kept part above the plane is integrated in closed
+                // form; +R to cell a, -R to cell a-1.
+                __syncwarp();
+                int pre2 = k;
+                for (int o = 1; o < 32; o <<= 1) {
+                    int y = __shfl_up_sync(0xffffffffu, pre2, o);
+                    if (lane >= o) pre2 += y;
+                }
+                const int total2 = __shfl_sync(0xffffffffu, pre2, 31);
+                pre2 -= k;
+                for (int eb = 0; eb < total2; eb += 32) {
+                    const int e = eb + lane;
+                    int src = 0;
+#pragma unroll
+                    for (int step = 16; step; step >>= 1) {
+                        int probe = __shfl_sync(0xffffffffu, pre2, src + step);
+                        if (probe <= e) src += step;
+                    }
+                    const int s_pre = __shfl_sync(0xffffffffu, pre2, src);
+                    const unsigned int s_order = __shfl_sync(0xffffffffu, f_order, src);
+                    const unsigned int s_info = __shfl_sync(0xffffffffu, f_info, src);
+                    const int s_afirst = __shfl_sync(0xffffffffu, f_afirst, src);
+                    const double s_w = __shfl_sync(0xffffffffu, f_w, src);
+                    if (e < total2) {
+                        const int a = s_afirst + (e - s_pre);
+                        const int colofs = s_info & 511, ax = (s_info >> 9) & 3;
+                        const int c_lo = (s_info >> 11) & 7, c_hi = (s_info >> 14) & 7, n = (s_info >> 17) & 7;
+                        const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
+                        PolyBuf<32> qs{wpoly + src};
+                        const double R = plane_integral6<32>(qs, s_order, n, (double)a) * (1.0 / 6.0) * s_w;
+                        if (COUNT) cnt.plane_evals++;
+                        if (R != 0.0) {
+                            if (a <= c_hi) { atomicAdd(acc + colofs + a * su, R); if (COUNT) cnt.cells++; }
+                            if (a - 1 >= c_lo) { atomicAdd(acc + colofs + (a - 1) * su, -R); if (COUNT) cnt.cells++; }
+                        }
+                    }
+                }
+                __syncwarp();
             }
         }
     }
