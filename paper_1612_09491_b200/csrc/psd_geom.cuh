@@ -203,9 +203,18 @@ struct PolyBuf {
 // (`fresh`), so 3 + 4 walls = 7 slots suffice (POLY_CAP = 8).
 struct PolyRef {
     unsigned order;
+    unsigned oc;  // nibble i = outcode of vertex i: bit k set = inside wall k (0: v>=0, 1: v<=1, 2: w>=0, 3: w<=1)
     int n;
     int fresh;
 };
+
+// bit k of every nibble of x (7 nibbles) gathered into bits 0..6
+__device__ __forceinline__ unsigned gather_nibble_bit(unsigned x, int k) {
+    unsigned y = (x >> k) & 0x01111111u;
+    y = (y | (y >> 3)) & 0x03030303u;
+    y = (y | (y >> 6)) & 0x000f000fu;
+    return (y | (y >> 12)) & 0x7fu;
+}
 
 __device__ __forceinline__ int slot_of(unsigned order, int i) { return (order >> (4 * i)) & 7; }
 __device__ __forceinline__ unsigned nib_mask(int n) { return n >= 8 ? 0xffffffffu : ((1u << (4 * n)) - 1u); }
@@ -228,11 +237,7 @@ template <int S>
 __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
     const int ax = 1 + (wall >> 1);
     const bool up = wall & 1;
-    unsigned mask = 0;
-    for (int i = 0; i < r.n; ++i) {
-        const double x = q.at(slot_of(r.order, i), ax);
-        mask |= (unsigned)((up ? 1.0 - x : x) >= 0.0) << i;
-    }
+    const unsigned mask = gather_nibble_bit(r.oc, wall);
     const unsigned full = (1u << r.n) - 1u;
     if (mask == full) return;
     if (mask == 0) { r.n = 0; return; }
@@ -269,7 +274,15 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
     // order: X_in, the inside run (starting at i_in), X_out
     const int m = __popc(mask);
     const unsigned rot = i_in ? ((r.order >> (4 * i_in)) | (r.order << (4 * (r.n - i_in)))) : r.order;
+    const unsigned roc = i_in ? ((r.oc >> (4 * i_in)) | (r.oc << (4 * (r.n - i_in)))) : r.oc;
+    // outcodes of the new points: on this wall and inside the opposite one; the other axis by compare
+    const unsigned own = ax == 1 ? 3u : 12u;
+    const double yo = ax == 1 ? xo[2] : xo[1], yi = ax == 1 ? xi[2] : xi[1];
+    const int sh = ax == 1 ? 2 : 0;
+    const unsigned oc_out = own | ((unsigned)(yo >= 0.0) | (unsigned)(yo <= 1.0) << 1) << sh;
+    const unsigned oc_in = own | ((unsigned)(yi >= 0.0) | (unsigned)(yi <= 1.0) << 1) << sh;
     r.order = (unsigned)s_in | ((rot & nib_mask(m)) << 4) | ((unsigned)s_out << (4 * (m + 1)));
+    r.oc = oc_in | ((roc & nib_mask(m)) << 4) | (oc_out << (4 * (m + 1)));
     r.n = m + 2;
 }
 
@@ -344,17 +357,18 @@ template <int S>
 __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     FaceClip fc;
     fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.umin = fc.umax = 0.0;
-    double minv = 1e300, maxv = -1e300, minw = 1e300, maxw = -1e300;
+    unsigned oc = 0, all_in = 15u, any_in = 0u;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
-        double v = q.at(i, 1), w = q.at(i, 2);
-        minv = fmin(minv, v); maxv = fmax(maxv, v);
-        minw = fmin(minw, w); maxw = fmax(maxw, w);
+        const double v = q.at(i, 1), w = q.at(i, 2);
+        const unsigned o = (unsigned)(v >= 0.0) | (unsigned)(v <= 1.0) << 1 | (unsigned)(w >= 0.0) << 2 |
+                           (unsigned)(w <= 1.0) << 3;
+        oc |= o << (4 * i);
+        all_in &= o; any_in |= o;
     }
-    if (maxv <= 0.0 || minv >= 1.0 || maxw <= 0.0 || minw >= 1.0) return fc;
-    PolyRef r{0x210u, 3, 3};
-    unsigned pending = (unsigned)(minv < 0.0) | (unsigned)(maxv > 1.0) << 1 | (unsigned)(minw < 0.0) << 2 |
-                       (unsigned)(maxw > 1.0) << 3;
+    if (any_in != 15u) return fc;  // all three vertices outside one wall
+    PolyRef r{0x210u, oc, 3, 3};
+    unsigned pending = all_in ^ 15u;
     while (pending && r.n) {
         const int wall = __ffs(pending) - 1;
         pending &= pending - 1;

@@ -317,10 +317,9 @@ struct DepositArgs {
 
 constexpr int DEP_WARPS = 4;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
-constexpr int POLY_SLOTS = 7;  // triangle + one fresh slot per column wall
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
-// [3*POLY_SLOTS][32], private column [8][32], slot words [32] (u32)
-constexpr int WARP_SCRATCH = (13 + 3 * POLY_SLOTS + TILE) * 32 + 16;
+// [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32)
+constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP) * 32 + 32 + 16;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
 
 __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile, int& level,
@@ -344,26 +343,22 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
 }
 
 // One CTA per work item (a chunk of one tile's pair list), an 8^3 fp64 accumulator in shared
-// memory.  Each warp fetches 32 pairs at a time:
+// memory.  Each warp takes 32 pairs at a time:
 //   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
-//            into the warp's slots; the rectangle of columns its range meets inside the tile.
-//   stage B  the column jobs (slot, column) of the 32 slots are numbered by a warp prefix sum;
-//            lane = job, 32 jobs at a time, so a large tet fans its columns across the lanes
-//            and small tets pack several per warp.
-//   stage C  the job runs the 4 faces of its tet in turn (the same face in every lane): wall
-//            clip, trivial cells, cutting planes, all added to the lane's PRIVATE column of 8
-//            cells (no atomics; the +A / -A shares of upper and lower faces below the tet
-//            cancel there); then the column is added to the tile, one atomic per non-empty cell.
+//            into the warp's slots; per face the rectangle of columns its projection meets.
+//   stage B  the face jobs (slot, face, column) of the 32 slots are numbered by a warp prefix
+//            sum of the rectangle sizes; lane = job, 32 jobs at a time, every lane busy.
+//   stage C  face_job: wall clip, closed-form plane integrals, shares added to the tile (a4-a6).
 // The tile is flushed to global memory with fp64 reductions at the end (a6).
 template <bool COUNT>
 __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                            // [13][32]
-    double* wpoly = wtet + 13 * 32;                                                     // [21][32]
-    double* wcol = wpoly + 3 * POLY_SLOTS * 32 + lane;                                  // [8][32]
-    unsigned int* wword = reinterpret_cast<unsigned int*>(wpoly + (3 * POLY_SLOTS + TILE) * 32);  // [32]
+    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
+    double* wpoly = wtet + 13 * 32;                                                    // [24][32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * POLY_CAP * 32);  // [32]
+    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 32);                 // [32]
     PolyBuf<32> poly{wpoly + lane};
 
     const Item item = A.items[blockIdx.x];
@@ -406,22 +401,33 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
         int my_images = have ? nimg[0] * nimg[1] * nimg[2] : 0;
         const int max_images = __reduce_max_sync(0xffffffffu, my_images);
         for (int img = 0; img < max_images; ++img) {
-            // ---- stage A: slot = lane.  Tile-local vertices, weight, column rectangle.
-            int njobs = 0;
+            // ---- stage A: slot = lane.  Tile-local vertices, weight, face rectangles.
+            unsigned int cnts = 0u;  // face jobs of this slot, 8 bits per face
             __syncwarp();
             if (img < my_images) {
                 int m[3] = {mlo[0] + img % nimg[0], mlo[1] + (img / nimg[0]) % nimg[1],
                             mlo[2] + img / (nimg[0] * nimg[1])};
                 int lo[3], hi[3];
+                double gl[4][3];
 #pragma unroll
                 for (int x = 0; x < 3; ++x) {
                     int o = org[x] + m[x] * Gl;
                     lo[x] = max(t.lo[x] - o, 0);
                     hi[x] = min(t.hi[x] - o, TILE - 1);
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) wtet[(3 * v + x) * 32 + lane] = t.g[v][x] - (double)o;
+                    for (int v = 0; v < 4; ++v) {
+                        gl[v][x] = t.g[v][x] - (double)o;
+                        wtet[(3 * v + x) * 32 + lane] = gl[v][x];
+                    }
                 }
                 wtet[12 * 32 + lane] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
+                int ax = A.chord_axis;
+                if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
+                    int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
+                    ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
+                }
+                const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
+                unsigned long long rect = 0ull;
                 if (det == 0.0) {  // degenerate: whole mass to the centroid cell (Q6)
                     if (A.weight_mode == 0) {
                         int c[3];
@@ -434,25 +440,49 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                         }
                         if (in) atomicAdd(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], A.mass_per_tet);
                     }
-                    wword[lane] = 0u;
                 } else {
-                    int ax = A.chord_axis;
-                    if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
-                        int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
-                        ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
+                        double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300, mxu = -1e300;
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            if (v == f) continue;
+                            // av, aw, ax are runtime: select instead of indexing
+                            double cu = ax == 0 ? gl[v][0] : (ax == 1 ? gl[v][1] : gl[v][2]);
+                            double cv = av == 0 ? gl[v][0] : (av == 1 ? gl[v][1] : gl[v][2]);
+                            double cw = aw == 0 ? gl[v][0] : (aw == 1 ? gl[v][1] : gl[v][2]);
+                            mnv = fmin(mnv, cv); mxv = fmax(mxv, cv);
+                            mnw = fmin(mnw, cw); mxw = fmax(mxw, cw);
+                            mxu = fmax(mxu, cu);
+                        }
+                        const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
+                        const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
+                        const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
+                        const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
+                        const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                        // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
+                        const int v0 = max(__double2int_rd(mnv), lov), v1 = min(__double2int_ru(mxv) - 1, hiv);
+                        const int w0 = max(__double2int_rd(mnw), low), w1 = min(__double2int_ru(mxw) - 1, hiw);
+                        int c = 0;
+                        if (v1 >= v0 && w1 >= w0 && mxu > (double)lou) {
+                            c = (v1 - v0 + 1) * (w1 - w0 + 1);
+                            rect |= (unsigned long long)(v0 | (v1 - v0) << 3 | w0 << 6 | (w1 - w0) << 9) << (16 * f);
+                        }
+                        cnts |= (unsigned int)c << (8 * f);
                     }
-                    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-                    const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
-                    const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
-                    const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
-                    const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
-                    const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
-                    const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
-                    njobs = (hiv - lov + 1) * (hiw - low + 1);
-                    wword[lane] = (unsigned)(ax | lou << 2 | hiu << 5 | lov << 8 | low << 11 | (hiw - low) << 14);
                 }
+                const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
+                wrect[lane] = rect;
+                wword[lane] = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
-            // ---- stage B: exclusive prefix of the job counts over the 32 slots
+            // ---- stage B: one pass per face (jobs of one pass never share a (tet, cell), so the
+            // shared atomics of a pass collide only between different tets); exclusive prefix of
+            // the face's job counts over the 32 slots
+            __syncwarp();
+#pragma unroll 1
+            for (int f = 0; f < 4; ++f) {
+            const int njobs = (cnts >> (8 * f)) & 255;
             int pre = njobs;
             for (int o = 1; o < 32; o <<= 1) {
                 int y = __shfl_up_sync(0xffffffffu, pre, o);
@@ -460,7 +490,6 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
             }
             const int total = __shfl_sync(0xffffffffu, pre, 31);
             pre -= njobs;
-            __syncwarp();
             for (int jb = 0; jb < total; jb += 32) {
                 const int job = jb + lane;
                 int slot = 0;  // largest slot with pre[slot] <= job
@@ -470,62 +499,97 @@ __global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A)
                     if (probe <= job) slot += step;
                 }
                 const int spre = __shfl_sync(0xffffffffu, pre, slot);
+                // ---- stage C1: lane = face job.  Wall clip; the polygon stays in the lane's buffer.
+                unsigned int f_order = 0, f_info = 0;
+                int f_afirst = 0, k = 0;
+                double f_w = 0.0;
                 if (job < total) {
-                    // ---- decode (slot, column)
+                    // decode (slot, column)
                     const unsigned int word = wword[slot];
                     const int local = job - spre;
-                    const int nw = ((word >> 14) & 7) + 1;
-                    const int cv = ((word >> 8) & 7) + local / nw, cw = ((word >> 11) & 7) + local % nw;
+                    const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
+                    const int nw = ((r16 >> 9) & 7) + 1;
+                    const int cv = (r16 & 7) + local / nw, cw = ((r16 >> 6) & 7) + local % nw;
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
+                    // the face triangle, column-local, into slots 0..2 of the lane's polygon buffer
                     const double* ts = wtet + slot;
+                    const unsigned int fv = FACE_TABLE >> (6 * f);
                     const double ov = (double)cv, ow = (double)cw;
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) {
+                        const int vi = (fv >> (2 * i)) & 3;
+                        poly.at(i, 0) = ts[(3 * vi + ax) * 32];
+                        poly.at(i, 1) = ts[(3 * vi + av) * 32] - ov;
+                        poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
+                    }
+                    f_w = ts[12 * 32];
                     if (COUNT) cnt.jobs++;
-#pragma unroll
-                    for (int c = 0; c < TILE; ++c) wcol[c * 32] = 0.0;
-                    int c_first = c_hi + 1;  // lowest cell any face reaches with a non-cancelling share
-                    // ---- stage C: the 4 faces in turn
-#pragma unroll 1
-                    for (int f = 0; f < 4; ++f) {
-                        const unsigned int fv = FACE_TABLE >> (6 * f);
-#pragma unroll
-                        for (int i = 0; i < 3; ++i) {
-                            const int vi = (fv >> (2 * i)) & 3;
-                            poly.at(i, 0) = ts[(3 * vi + ax) * 32];
-                            poly.at(i, 1) = ts[(3 * vi + av) * 32] - ov;
-                            poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
-                        }
-                        const FaceClip fc = face_clip<32>(poly);
-                        if (fc.n >= 3 && fc.umax <= (double)c_lo) c_first = c_lo;  // a face below the run: nothing cancels
-                        if (fc.n >= 3 && fc.umax > (double)c_lo) {
-                            if (COUNT) cnt.face_clips++;
-                            const FaceRun fr = face_run(fc, c_lo, c_hi);
-                            c_first = min(c_first, max(fr.a_first - 1, c_lo));
-                            for (int c = c_lo; c <= fr.t_hi; ++c)
-                                wcol[c * 32] += (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
-                            for (int a = fr.a_first; a <= fr.a_last; ++a) {
-                                const double R = plane_integral6<32>(poly, fc.order, fc.n, (double)a) * (1.0 / 6.0);
-                                if (COUNT) cnt.plane_evals++;
-                                if (a <= c_hi) wcol[a * 32] += R;
-                                if (a - 1 >= c_lo) wcol[(a - 1) * 32] -= R;
+                    const FaceClip fc = face_clip<32>(poly);
+                    if (fc.n >= 3 && fc.umax > (double)c_lo) {
+                        if (COUNT) cnt.face_clips++;
+                        const FaceRun fr = face_run(fc, c_lo, c_hi);
+                        // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
+                        const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
+                        const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
+                        const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
+                        const int colofs = cv * sv + cw * sw;
+                        // trivial part: cells entirely below Q get its projected area, the cell
+                        // holding umin gets M1 - c A
+                        for (int c = c_lo; c <= fr.t_hi; ++c) {
+                            const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
+                            if (D != 0.0) {
+                                atomicAdd(acc + colofs + c * su, f_w * D);
+                                if (COUNT) cnt.cells++;
                             }
                         }
+                        k = max(fr.a_last - fr.a_first + 1, 0);
+                        f_order = fc.order;
+                        f_afirst = fr.a_first;
+                        f_info = (unsigned)colofs | (unsigned)ax << 9 | (unsigned)c_lo << 11 | (unsigned)c_hi << 14 |
+                                 (unsigned)fc.n << 17;
                     }
-                    // ---- the column into the tile: cells below c_first hold only the cancelled
-                    // +A/-A shares of the faces above them
-                    const double w = ts[12 * 32];
-                    const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
-                    const int sv = av == 0 ? 64 : (av == 1 ? 8 : 1);
-                    const int sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
-                    double* col = acc + cv * sv + cw * sw;
-                    for (int c = c_first; c <= c_hi; ++c) {
-                        const double v = wcol[c * 32];
-                        if (v != 0.0) {
-                            atomicAdd(col + c * su, w * v);
-                            if (COUNT) cnt.cells++;
+                }
+                // ---- stage C2: the cutting planes (polygon, a) of the 32 jobs, numbered by a warp
+                // prefix sum; lane = plane.  The kept part above the plane is integrated in closed
+                // form; +R to cell a, -R to cell a-1.
+                __syncwarp();
+                int pre2 = k;
+                for (int o = 1; o < 32; o <<= 1) {
+                    int y = __shfl_up_sync(0xffffffffu, pre2, o);
+                    if (lane >= o) pre2 += y;
+                }
+                const int total2 = __shfl_sync(0xffffffffu, pre2, 31);
+                pre2 -= k;
+                for (int eb = 0; eb < total2; eb += 32) {
+                    const int e = eb + lane;
+                    int src = 0;
+#pragma unroll
+                    for (int step = 16; step; step >>= 1) {
+                        int probe = __shfl_sync(0xffffffffu, pre2, src + step);
+                        if (probe <= e) src += step;
+                    }
+                    const int s_pre = __shfl_sync(0xffffffffu, pre2, src);
+                    const unsigned int s_order = __shfl_sync(0xffffffffu, f_order, src);
+                    const unsigned int s_info = __shfl_sync(0xffffffffu, f_info, src);
+                    const int s_afirst = __shfl_sync(0xffffffffu, f_afirst, src);
+                    const double s_w = __shfl_sync(0xffffffffu, f_w, src);
+                    if (e < total2) {
+                        const int a = s_afirst + (e - s_pre);
+                        const int colofs = s_info & 511, ax = (s_info >> 9) & 3;
+                        const int c_lo = (s_info >> 11) & 7, c_hi = (s_info >> 14) & 7, n = (s_info >> 17) & 7;
+                        const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
+                        PolyBuf<32> qs{wpoly + src};
+                        const double R = plane_integral6<32>(qs, s_order, n, (double)a) * (1.0 / 6.0) * s_w;
+                        if (COUNT) cnt.plane_evals++;
+                        if (R != 0.0) {
+                            if (a <= c_hi) { atomicAdd(acc + colofs + a * su, R); if (COUNT) cnt.cells++; }
+                            if (a - 1 >= c_lo) { atomicAdd(acc + colofs + (a - 1) * su, -R); if (COUNT) cnt.cells++; }
                         }
                     }
                 }
+                __syncwarp();
+            }
             }
         }
     }
