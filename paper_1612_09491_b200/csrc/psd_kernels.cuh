@@ -315,6 +315,9 @@ struct DepositArgs {
     unsigned long long* stats;
 };
 
+#ifndef DEP_MIN_CTAS
+#define DEP_MIN_CTAS 4
+#endif
 constexpr int DEP_WARPS = 4;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
@@ -351,7 +354,7 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
 //   stage C  face_job: wall clip, closed-form plane integrals, shares added to the tile (a4-a6).
 // The tile is flushed to global memory with fp64 reductions at the end (a6).
 template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, 4) k_deposit_tiles(DepositArgs A) {
+__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

@@ -326,3 +326,83 @@ def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_win, edg
     ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
     ctx.psd_deposit_uniform(G, grid)
     assert float((grid - 1.0).abs().max()) < 1e-9
+
+
+def test_cfg3_full_size_patches(psd, ctx, oracle):
+    """BASELINE.json configs[3]: 256^3 particles, base 128^3 in 16^3-cell patches, 2 levels,
+    factor 4 (rule: DESIGN.md Q14).  Refinement census and patch list bit-exact vs the oracle,
+    deposit parity on sampled patches of every level, and the properties that hold for all of
+    them: level 0 carries the whole mass, a refined coarse cell equals the sum of its 8 children."""
+    import torch
+    cfg = psd_inputs.CONFIGS[3]
+    pc = cfg["patches"]
+    base_G, P, max_level, factor = pc["base_G"], pc["P"], pc["max_level"], pc["factor"]
+    pos = psd_inputs.config_positions(3)
+    ctx.psd_build_tets(to_dev(pos))
+    patches, counts = ctx.psd_refine_patches(base_G, P, max_level, factor, want_counts=True)
+    ocounts = [oracle.patch_counts(pos, 1.0, base_G, P, l) for l in range(max_level + 1)]
+    for a, b in zip(counts, ocounts):
+        assert np.array_equal(a, b)
+    assert np.array_equal(patches, oracle.refine_patches(ocounts, factor))
+    levels = patches[:, 0]
+    assert (levels == 0).sum() == (base_G // P) ** 3
+    assert (levels == 1).any() and (levels == 2).any(), "the refinement rule must fire on cfg3"
+    lit = ctx.psd_refine_patches(base_G, P, max_level, factor, rule=psd.RULE_LITERAL_TOP_DOWN)
+    assert np.array_equal(lit, oracle.refine_patches(ocounts, factor, oracle.RULE_LITERAL_TOP_DOWN))
+    mass = ctx.psd_deposit_patches(patches, P, base_G)
+    s = ctx.psd_get_stats()
+    assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    assert_mass(mass[torch.from_numpy(levels == 0).cuda()].sum())
+    # sampled patches, two per level (seeded), against the oracle
+    pick = []
+    for l in range(max_level + 1):
+        idx = np.nonzero(levels == l)[0]
+        u = psd_inputs.splitmix64(3000 + l, 0, 2) % np.uint64(len(idx))
+        pick += [int(idx[int(x)]) for x in u]
+    ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches[pick])
+    got = mass[torch.tensor(pick, device="cuda")].cpu().numpy()
+    mx = float(mass.max())
+    err = np.abs(got - ora)
+    assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), float(err.max())
+    # restriction (Q13): every refined patch's coarse cells equal the sum of the 8 children
+    index = {tuple(r): i for i, r in enumerate(patches.tolist())}
+    checked = 0
+    for i, (l, ox, oy, oz) in enumerate(patches.tolist()):
+        if l == max_level or (l + 1, 2 * ox, 2 * oy, 2 * oz) not in index or checked >= 40:
+            continue
+        coarse = mass[i]
+        fine = torch.empty((2 * P, 2 * P, 2 * P), dtype=torch.float64, device="cuda")
+        for d in range(8):
+            a, b, c = d & 1, (d >> 1) & 1, d >> 2
+            fine[a * P:(a + 1) * P, b * P:(b + 1) * P, c * P:(c + 1) * P] = \
+                mass[index[(l + 1, 2 * ox + a, 2 * oy + b, 2 * oz + c)]]
+        summed = fine.reshape(P, 2, P, 2, P, 2).sum(dim=(1, 3, 5))
+        assert float((summed - coarse).abs().max()) <= 1e-9 * mx
+        checked += 1
+    assert checked > 0
+
+
+def test_cfg4_full_size_uniform(psd, ctx, oracle):
+    """BASELINE.json configs[4]: 512^3 particles (805 M tets) onto 1024^3 cells (8.6 GB) in one
+    pass: total mass, positivity, oracle parity on sampled windows, signed-volume cover."""
+    import torch
+    cfg = psd_inputs.CONFIGS[4]
+    G = cfg["G"]
+    pos = psd_inputs.config_positions(4)
+    ctx.psd_build_tets(to_dev(pos))
+    grid = torch.empty((G, G, G), dtype=torch.float64, device="cuda")
+    ctx.psd_deposit_uniform(G, grid)
+    s = ctx.psd_get_stats()
+    assert s.n_tets == 6 * cfg["N"] ** 3 == 805306368 and s.n_degenerate == 0
+    total = float(grid.sum())
+    assert abs(total - 1.0) <= 1e-10, total
+    assert float(grid.min()) > 0.0
+    mx = float(grid.max())
+    edge = 8
+    for lo in [(G - 3, 5, G - 6), (417, 230, 771)]:
+        ora = oracle.deposit_window(pos, 1.0, 1.0, G, lo, (edge,) * 3)
+        err = np.abs(window_of(grid, lo, edge, G) - ora)
+        assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (lo, float(err.max()))
+    ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
+    ctx.psd_deposit_uniform(G, grid)
+    assert float((grid - 1.0).abs().max()) < 1e-9
