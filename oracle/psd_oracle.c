@@ -288,8 +288,8 @@ static void deposit_tet(const tet_t *t, double m, int mode, const target_t *T, i
         for (int64_t cy = t->lo[1]; cy <= t->hi[1]; ++cy)
             for (int64_t cz = t->lo[2]; cz <= t->hi[2]; ++cz) {
                 double *cell = target_cell(T, cx, cy, cz);
+                if (!cell) continue; /* outside the window / patch */
                 if (n_cand) ++*n_cand;
-                if (!cell) continue;
                 int64_t c[3] = {cx, cy, cz};
                 REAL vol = tet_cell_volume(t->g, c);
                 if (vol != 0 && n_nonzero) ++*n_nonzero;
@@ -521,9 +521,11 @@ void psdo_kuhn_table(int *out24) {
  * patch receives the full deposit of every tet overlapping it.                        */
 typedef struct { int32_t level, ox, oy, oz; } psdo_patch;
 
-int psdo_deposit_patches(const void *pos, int dtype, int stride, int N, double L, double M,
-                         int base_G, int P, const psdo_patch *patches, int64_t n_patch,
-                         double *mass, int mode) {
+/* per_patch (optional): [q*2+0] candidate cells, [q*2+1] cells with non-zero overlap of patch q
+ * (counters only; the arithmetic is that of psdo_deposit_patches). */
+int psdo_deposit_patches_stats(const void *pos, int dtype, int stride, int N, double L, double M,
+                               int base_G, int P, const psdo_patch *patches, int64_t n_patch,
+                               double *mass, int mode, int64_t *per_patch) {
     if (N < 2 || base_G < 1 || P < 1 || base_G % P) return 1;
     memset(mass, 0, sizeof(double) * (size_t)(n_patch * P * P * P));
     int rc = 0;
@@ -534,9 +536,18 @@ int psdo_deposit_patches(const void *pos, int dtype, int stride, int N, double L
         int64_t wn[3] = {P, P, P};
         target_t T = {G, mass + q * (int64_t)P * P * P, 1, {wlo[0], wlo[1], wlo[2]},
                       {wn[0], wn[1], wn[2]}};
-        rc |= deposit_common(pos, dtype, stride, N, L, M, (int)G, &T, mode, NULL);
+        int64_t st[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        rc |= deposit_common(pos, dtype, stride, N, L, M, (int)G, &T, mode, st);
+        if (per_patch) { per_patch[2 * q] = st[1]; per_patch[2 * q + 1] = st[2]; }
     }
     return rc;
+}
+
+int psdo_deposit_patches(const void *pos, int dtype, int stride, int N, double L, double M,
+                         int base_G, int P, const psdo_patch *patches, int64_t n_patch,
+                         double *mass, int mode) {
+    return psdo_deposit_patches_stats(pos, dtype, stride, N, L, M, base_G, P, patches, n_patch, mass,
+                                      mode, NULL);
 }
 
 /* counts[l] is a dense (base_G/P * 2^l)^3 array: number of tets whose cell range on the

@@ -219,6 +219,24 @@ def deposit_patches(pos, L, M, base_G: int, P: int, patches, mode: int = MODE_MA
     return mass
 
 
+def deposit_patches_stats(pos, L, M, base_G: int, P: int, patches):
+    """deposit_patches plus per-patch counters: (masses, (n,2) int64 [candidate cells, cells with
+    non-zero overlap]) -- the method-defined counts bench.py's work model uses."""
+    p, dt, stride, N = _pos_args(pos)
+    pa = np.ascontiguousarray(patches, dtype=np.int32).reshape(-1, 4)
+    n = pa.shape[0]
+    mass = np.empty((n, P, P, P), dtype=np.float64)
+    st = np.zeros((n, 2), dtype=np.int64)
+    lib = _lib()
+    lib.psdo_deposit_patches_stats.argtypes = list(lib.psdo_deposit_patches.argtypes) + [C.POINTER(C.c_int64)]
+    rc = lib.psdo_deposit_patches_stats(p, dt, stride, N, L, M, base_G, P,
+                                        pa.ctypes.data_as(C.POINTER(_Patch)), n, _dp(mass), MODE_MASS,
+                                        _i64p(st))
+    if rc:
+        raise ValueError("psdo_deposit_patches_stats: invalid argument")
+    return mass, st
+
+
 def patch_counts(pos, L, base_G: int, P: int, level: int) -> np.ndarray:
     """#tets whose cell range meets each candidate patch position of `level`."""
     p, dt, stride, N = _pos_args(pos)
