@@ -163,7 +163,8 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                     long long id = tile_id_of(s, level, tx, ty, tz);
                     if (id < 0) return;
                     if (!SCATTER) {
-                        atomicAdd(&tile_counts[id], 1u);
+                        const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)id);
+                        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&tile_counts[id], (unsigned int)__popc(peers));
                         atomicAdd(&sh_stat[ST_PAIRS], 1ull);
                         atomicAdd(&sh_hist[1][bit_width_u64((unsigned long long)(inside - 1))], 1u);
                     } else {
@@ -732,8 +733,12 @@ __global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, i
     load_tet_vertices(p, id / 6, (int)(id % 6), V);
     Tet t;
     finish_tet(V, __ddiv_rn((double)Gl, p.L), t);
+    // neighbouring tets mostly meet the same positions: one atomic per distinct position among the
+    // lanes that are here together
     for_each_block(t.lo, t.hi, Gl, P, np, [&](int bx, int by, int bz, long long) {
-        atomicAdd(&counts[((long long)bx * np + by) * np + bz], 1ull);
+        const unsigned int key = (unsigned int)(((long long)bx * np + by) * np + bz);
+        const unsigned int peers = __match_any_sync(__activemask(), key);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&counts[key], (unsigned long long)__popc(peers));
     });
 }
 
