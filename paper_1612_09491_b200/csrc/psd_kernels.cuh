@@ -319,7 +319,10 @@ struct DepositArgs {
 #ifndef DEP_MIN_CTAS
 #define DEP_MIN_CTAS 4
 #endif
-constexpr int DEP_WARPS = 4;
+#ifndef DEP_WARPS_N
+#define DEP_WARPS_N 4
+#endif
+constexpr int DEP_WARPS = DEP_WARPS_N;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
 // [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32)

@@ -78,3 +78,10 @@ def test_reference_arm_other_ranks_exit_without_work():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
                         "--gpus", "2"], capture_output=True, text=True, timeout=120, env=env)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_roofline_traffic_comes_from_the_committed_capture():
+    import bench
+    v = bench.read_ncu_traffic("cfg1_128_256", "k_deposit_tiles")
+    assert isinstance(v, int) and v > 100e6
+    assert bench.read_ncu_traffic("no_such_workload", "k_deposit_tiles") is None

@@ -406,3 +406,35 @@ def test_cfg4_full_size_uniform(psd, ctx, oracle):
     ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
     ctx.psd_deposit_uniform(G, grid)
     assert float((grid - 1.0).abs().max()) < 1e-9
+
+
+# ------------------------------------------------------------------ SURVEY.md 8(f) row 1
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_paper_weak_scaling_workload_jittered_lattice(psd, ctx, oracle, kernel):
+    """PAPER.md:175 (section 7.2): lattice + independent uniform offsets of up to one cell width,
+    deposited on a grid with G = N/2, so most tets fall inside one or two cells: the trivial /
+    accumulate path instead of the clip path.  Every cell against the oracle."""
+    N, G = 32, 16
+    pos = psd_inputs.jittered_lattice(N, seed=175, amplitude_cells=1.0)
+    ora, st = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(G)
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora, what="jittered lattice")
+    s = ctx.psd_get_stats()
+    assert s.n_inverted == st["n_inverted"] > 0 and s.sum_cells == st["n_candidates"]
+
+
+@pytest.mark.parametrize("N", [2, 3])
+def test_minimal_lattice_and_single_tile(psd, ctx, oracle, N):
+    """Smallest inputs the ABI accepts, one 8^3 tile.  N = 2: every Lagrangian cell edge is about
+    L/2, outside the unwrap's validity (Q4) -- both sides must still take the same
+    minimum image, rint for rint.  N = 3: the smallest valid lattice."""
+    pos = psd_inputs.zeldovich_positions(N, 3, 1, 0.2, 5, dtype="float64", stride=3)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 8)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(8)
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora)
+    assert ctx.psd_get_stats().n_tiles == 1
