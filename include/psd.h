@@ -92,7 +92,8 @@ typedef struct {
     int64_t n_face_clips;   /* jobs whose clipped polygon is non-empty and reaches the run */
     int64_t n_plane_evals;  /* closed-form lattice-plane integrals of a face polygon     */
     int64_t n_cells_written;/* per-face cell shares added to accumulators                */
-    /* device pointer to the per-tile counts of the last binned deposit (n_tiles uint32) */
+    /* device pointer to the per-(tile, size class) pair counts of the last binned deposit
+       (2 * n_tiles uint32, see psd_get_tile_class_counts) */
     const uint32_t* tile_counts_dev;
     /* device time of the phases of the last deposit, ms (0 if not recorded)             */
     float ms_census, ms_scan, ms_scatter, ms_deposit, ms_total;
@@ -163,6 +164,11 @@ PSD_API int psd_get_stats(psd_ctx* ctx, psd_stats* out);
  * (tx*nt+ty)*nt+tz, nt = G/8.  Patches: patch-major, then the (P/8)^3 tiles of the patch.
  * PSD_ERR_STATE if the last deposit was not binned. */
 PSD_API int psd_get_tile_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap);
+
+/* As psd_get_tile_counts, split by the SIZE CLASS the pair lists are ordered by (BASELINE.json
+ * north_star: bins by tile and by cells touched): out_host[2*tile + 0] = pairs whose tet covers
+ * <= 8 cells of the tile ("small"), [2*tile + 1] = the others ("large"); cap >= 2 * n_tiles. */
+PSD_API int psd_get_tile_class_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap);
 
 PSD_API int psd_set_option(psd_ctx* ctx, int key, double value);
 PSD_API int psd_sync(psd_ctx* ctx);

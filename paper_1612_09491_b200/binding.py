@@ -19,7 +19,7 @@ RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN = 0, 1
 # every symbol include/psd.h declares (tests check the library exports exactly these)
 EXPORTS = ("psd_create", "psd_destroy", "psd_build_tets", "psd_deposit_uniform",
            "psd_refine_patches", "psd_deposit_patches", "psd_deposit_uniform_host",
-           "psd_get_stats", "psd_get_tile_counts", "psd_set_option", "psd_sync", "psd_last_error", "psd_launch_count",
+           "psd_get_stats", "psd_get_tile_counts", "psd_get_tile_class_counts", "psd_set_option", "psd_sync", "psd_last_error", "psd_launch_count",
            "psd_version")
 
 
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
     L.psd_deposit_uniform_host.argtypes = [vp, vp, i, i, i, d, d, i, vp]
     L.psd_get_stats.argtypes = [vp, C.POINTER(PsdStats)]
     L.psd_get_tile_counts.argtypes = [vp, C.POINTER(C.c_uint32), i64]
+    L.psd_get_tile_class_counts.argtypes = [vp, C.POINTER(C.c_uint32), i64]
     L.psd_set_option.argtypes = [vp, i, d]
     L.psd_sync.argtypes = [vp]
     L.psd_last_error.argtypes = [vp]
@@ -227,6 +228,13 @@ class Context:
 
     def psd_launch_count(self) -> int:
         return int(self._L.psd_launch_count(self._h))
+
+    def psd_get_tile_class_counts(self) -> np.ndarray:
+        """(n_tiles, 2) uint32: pairs of each tile by size class (small, large)."""
+        n = int(self.psd_get_stats().n_tiles)
+        out = np.zeros((max(n, 1), 2), dtype=np.uint32)
+        self._ck(self._L.psd_get_tile_class_counts(self._h, out.ctypes.data_as(C.POINTER(C.c_uint32)), 2 * n))
+        return out[:n]
 
     def psd_get_tile_counts(self) -> np.ndarray:
         n = int(self.psd_get_stats().n_tiles)

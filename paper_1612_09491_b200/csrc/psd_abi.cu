@@ -84,16 +84,17 @@ int reset_stats(psd_ctx* ctx) {
 int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     cudaStream_t st = ctx->stream;
     const long long ncell = (long long)ctx->part.N * ctx->part.N * ctx->part.N;
-    CK(ctx->tile_counts.ensure(sizeof(unsigned int) * n_tiles));
-    CK(ctx->cursors.ensure(sizeof(unsigned int) * n_tiles));
-    CK(ctx->tile_offsets.ensure(sizeof(unsigned long long) * (n_tiles + 1)));
-    CK(ctx->item_offsets.ensure(sizeof(unsigned long long) * (n_tiles + 1)));
-    const int nparts = (int)((n_tiles + SCAN_BLOCK - 1) / SCAN_BLOCK);
+    const long long n_bins = n_tiles * N_CLASSES;  // (tile, size class)
+    CK(ctx->tile_counts.ensure(sizeof(unsigned int) * n_bins));
+    CK(ctx->cursors.ensure(sizeof(unsigned int) * n_bins));
+    CK(ctx->tile_offsets.ensure(sizeof(unsigned long long) * (n_bins + 1)));
+    CK(ctx->item_offsets.ensure(sizeof(unsigned long long) * (n_bins + 1)));
+    const int nparts = (int)((n_bins + SCAN_BLOCK - 1) / SCAN_BLOCK);
     CK(ctx->part_pairs.ensure(sizeof(unsigned long long) * nparts));
     CK(ctx->part_items.ensure(sizeof(unsigned long long) * nparts));
     CK(ctx->totals.ensure(sizeof(unsigned long long) * 2));
-    CK(cudaMemsetAsync(ctx->tile_counts.p, 0, sizeof(unsigned int) * n_tiles, st));
-    CK(cudaMemsetAsync(ctx->cursors.p, 0, sizeof(unsigned int) * n_tiles, st));
+    CK(cudaMemsetAsync(ctx->tile_counts.p, 0, sizeof(unsigned int) * n_bins, st));
+    CK(cudaMemsetAsync(ctx->cursors.p, 0, sizeof(unsigned int) * n_bins, st));
     int rc = reset_stats(ctx);
     if (rc) return rc;
 
@@ -104,13 +105,13 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                           nullptr, nullptr, ctx->stats.as<unsigned long long>(),
                                           ctx->hist.as<unsigned long long>());
     CK(cudaEventRecord(ctx->ev[1], st));
-    k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk,
+    k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_bins, ctx->chunk,
                                                    ctx->part_pairs.as<unsigned long long>(),
                                                    ctx->part_items.as<unsigned long long>());
     k_scan_top<<<1, SCAN_BLOCK, 0, st>>>(ctx->part_pairs.as<unsigned long long>(),
                                          ctx->part_items.as<unsigned long long>(), nparts,
                                          ctx->totals.as<unsigned long long>());
-    k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk,
+    k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_bins, ctx->chunk,
                                                 ctx->part_pairs.as<unsigned long long>(),
                                                 ctx->part_items.as<unsigned long long>(),
                                                 ctx->tile_offsets.as<unsigned long long>(),
@@ -499,14 +500,30 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
     return PSD_OK;
 }
 
+int psd_get_tile_class_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap) {
+    if (!valid_ctx(ctx) || !out_host) return PSD_ERR_INVALID_ARG;
+    if (!ctx->binned_last || ctx->last.n_tiles <= 0) return fail(ctx, PSD_ERR_STATE, "no binned deposit to report");
+    const int64_t n_bins = ctx->last.n_tiles * N_CLASSES;
+    if (cap < n_bins) return fail(ctx, PSD_ERR_INVALID_ARG, "tile class count buffer too small");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(out_host, ctx->tile_counts.p, sizeof(uint32_t) * (size_t)n_bins, cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PSD_OK;
+}
+
 int psd_get_tile_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap) {
     if (!valid_ctx(ctx) || !out_host) return PSD_ERR_INVALID_ARG;
     if (!ctx->binned_last || ctx->last.n_tiles <= 0) return fail(ctx, PSD_ERR_STATE, "no binned deposit to report");
     if (cap < ctx->last.n_tiles) return fail(ctx, PSD_ERR_INVALID_ARG, "tile count buffer too small");
-    CK(cudaSetDevice(ctx->device));
-    CK(cudaMemcpyAsync(out_host, ctx->tile_counts.p, sizeof(uint32_t) * (size_t)ctx->last.n_tiles,
-                       cudaMemcpyDeviceToHost, ctx->stream));
-    CK(cudaStreamSynchronize(ctx->stream));
+    std::vector<uint32_t> bins((size_t)ctx->last.n_tiles * N_CLASSES);
+    int rc = psd_get_tile_class_counts(ctx, bins.data(), (int64_t)bins.size());
+    if (rc) return rc;
+    for (int64_t t = 0; t < ctx->last.n_tiles; ++t) {
+        uint32_t c = 0;
+        for (int k = 0; k < N_CLASSES; ++k) c += bins[(size_t)t * N_CLASSES + k];
+        out_host[t] = c;
+    }
     return PSD_OK;
 }
 

@@ -36,6 +36,12 @@ __device__ __forceinline__ int level_G(const Space& s, int level) {
 
 struct Item { unsigned int tile; unsigned int count; unsigned long long begin; };
 
+// a3: every tile's pair list is ordered by SIZE CLASS of the pair -- class 0 "small": the tet's
+// cell range covers <= 8 cells of the tile (buckets b <= 3 of the census histogram), class 1
+// "large" -- so the 32-pair batches a warp fetches hold tets of similar size.  Bin = tile * 2 + class.
+constexpr int N_CLASSES = 2;
+constexpr long long CLASS_SMALL_MAX_CELLS = 8;
+
 enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
        ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_COUNT };
 
@@ -162,14 +168,16 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                 for_each_block(t.lo, t.hi, Gl, TILE, nb, [&](int tx, int ty, int tz, long long inside) {
                     long long id = tile_id_of(s, level, tx, ty, tz);
                     if (id < 0) return;
+                    // size class of the pair: cells of the tet's range inside this tile (a3)
+                    const long long bin = id * N_CLASSES + (inside > CLASS_SMALL_MAX_CELLS ? 1 : 0);
                     if (!SCATTER) {
-                        const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)id);
-                        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&tile_counts[id], (unsigned int)__popc(peers));
+                        const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
+                        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&tile_counts[bin], (unsigned int)__popc(peers));
                         atomicAdd(&sh_stat[ST_PAIRS], 1ull);
                         atomicAdd(&sh_hist[1][bit_width_u64((unsigned long long)(inside - 1))], 1u);
                     } else {
-                        unsigned int slot = atomicAdd(&cursors[id], 1u);
-                        pair_ids[tile_offsets[id] + slot] = tet_id;
+                        unsigned int slot = atomicAdd(&cursors[bin], 1u);
+                        pair_ids[tile_offsets[bin] + slot] = tet_id;
                     }
                 });
             }
@@ -193,6 +201,17 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
 // second output: items per tile = ceil(count/chunk), scanned the same way.
 constexpr int SCAN_BLOCK = 1024;
 
+// work items of bin i: a tile's items are counted at its first bin (the chunks run over both
+// classes of the tile together), its other bins count none
+__device__ __forceinline__ unsigned long long bin_items(const unsigned int* counts, long long i, long long n,
+                                                        unsigned int chunk) {
+    if (i >= n || i % N_CLASSES != 0) return 0ull;
+    unsigned long long c = 0;
+#pragma unroll
+    for (int k = 0; k < N_CLASSES; ++k) c += counts[i + k];
+    return (c + chunk - 1) / chunk;
+}
+
 __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_partials(const unsigned int* counts, long long n,
                                                               unsigned int chunk,
                                                               unsigned long long* part_pairs,
@@ -200,7 +219,7 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_partials(const unsigned int
     __shared__ unsigned long long sp[32], si[32];
     long long i = blockIdx.x * (long long)SCAN_BLOCK + threadIdx.x;
     unsigned long long c = i < n ? counts[i] : 0ull;
-    unsigned long long it = (c + chunk - 1) / chunk;
+    unsigned long long it = bin_items(counts, i, n, chunk);
     for (int o = 16; o; o >>= 1) {
         c += __shfl_down_sync(0xffffffffu, c, o);
         it += __shfl_down_sync(0xffffffffu, it, o);
@@ -263,7 +282,7 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_final(const unsigned int* c
     __shared__ unsigned long long wp[32], wi[32];
     long long i = blockIdx.x * (long long)SCAN_BLOCK + threadIdx.x;
     unsigned long long a = i < n ? counts[i] : 0ull;
-    unsigned long long b = (a + chunk - 1) / chunk;
+    unsigned long long b = bin_items(counts, i, n, chunk);
     unsigned long long ia = a, ib = b;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (int o = 1; o < 32; o <<= 1) {
@@ -291,10 +310,12 @@ __global__ void __launch_bounds__(SCAN_BLOCK) k_scan_final(const unsigned int* c
 __global__ void k_items(const unsigned int* counts, long long n, unsigned int chunk,
                         const unsigned long long* tile_offsets,
                         const unsigned long long* item_offsets, Item* items) {
-    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;  // tile; n = number of tiles
     if (t >= n) return;
-    unsigned int c = counts[t];
-    unsigned long long io = item_offsets[t], po = tile_offsets[t];
+    unsigned int c = 0;
+#pragma unroll
+    for (int k = 0; k < N_CLASSES; ++k) c += counts[t * N_CLASSES + k];
+    unsigned long long io = item_offsets[t * N_CLASSES], po = tile_offsets[t * N_CLASSES];
     for (unsigned int done = 0; done < c; done += chunk) {
         Item it;
         it.tile = (unsigned int)t;

@@ -179,6 +179,12 @@ def test_census_bit_exact_with_images_and_inversions(psd, ctx, oracle):
         assert list(s.hist_tet) == cen["hist_tet"].tolist()
         assert list(s.hist_pair) == cen["hist_pair"].tolist()
         assert np.array_equal(ctx.psd_get_tile_counts(), cen["tile_counts"])
+        # size classes of the binning (a3): small = the tet's range covers <= 8 cells of the tile,
+        # i.e. buckets b <= 3 of the oracle's pair histogram
+        cls = ctx.psd_get_tile_class_counts().astype(np.int64)
+        assert np.array_equal(cls.sum(axis=1), cen["tile_counts"].astype(np.int64))
+        assert int(cls[:, 0].sum()) == int(cen["hist_pair"][:4].sum())
+        assert int(cls[:, 1].sum()) == int(cen["hist_pair"][4:].sum())
 
 
 @pytest.mark.parametrize("chunk", [32, 100, 1024])
