@@ -8,18 +8,20 @@
 // How (differs from the paper's K80 design):
 // the tet is kept as a boundary polytope (its 4 oriented faces).  The unit of work is a
 // FACE JOB: one face triangle against one COLUMN of cells (a unit square in two axes, running
-// along the third, "chord" axis u).  The triangle is clipped by the 4 axis-aligned walls of the
-// column (Sutherland-Hodgman, in place) giving a convex polygon Q, on which u is linear.  With
+// along the third, "chord" axis u).  The triangle is clipped by the (at most 4) axis-aligned walls
+// of the column it crosses -- a convex polygon meets a line on exactly two edges, so a clip is two
+// interpolations and a re-packed vertex order -- giving a convex polygon Q, on which u is linear.
+// With
 //     R_F(a) = signed integral over Q n {u >= a} of (u - a) dv dw
 // the divergence theorem (flux of (u-a,0,0)) gives, summed over the 4 faces,
 //     R(a) = vol(T n column n {u >= a}),
 // so the cell [a,a+1] receives R(a) - R(a+1): the cell's own faces never need a cap polygon
 // (column walls have zero u-flux and the cap u = a has u-a = 0), and every face adds its own
-// share to the cell independently of the other faces.  R_F(a) is evaluated in CLOSED FORM per
-// fan triangle of Q (the integral of (u-a)_+ over a triangle is a cubic in a between its sorted
-// vertex heights), so a lattice plane costs a few flops, not another clip.  All interpolation
-// is between points on opposite sides of a plane (convex combinations), every ratio used is in
-// [0,1], coordinates are local to the tile/column, arithmetic is fp64.
+// share to the cell independently of the other faces.  R_F(a) = M1 - a A below Q, 0 above it, and
+// for a plane that cuts Q the part above the plane is fanned from its first crossing with the
+// plane (plane_integral6): a sum of same-signed terms, a few flops per vertex, not another stored
+// clip.  All interpolation is between points on opposite sides of a plane (convex combinations),
+// every ratio used is in [0,1], coordinates are local to the tile/column, arithmetic is fp64.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

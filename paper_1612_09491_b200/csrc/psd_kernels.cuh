@@ -1,7 +1,7 @@
 // psd_kernels.cuh -- kernels of the deposit path (sm_100a).  Steps:
-//   a1 tet generation        load_tet_vertices / k_census / k_scatter / k_deposit_*
-//   a2 AABB + census         k_census      (per-tile counts, size-class histograms)
-//   a3 bin / sort            k_scan_* + k_scatter (counting sort of tet ids by tile) + k_items
+//   a1 tet generation        load_tet_vertices, inlined in k_census / k_deposit_* (nothing stored per tet)
+//   a2 AABB + census         k_census<false> (pair counts per (tile, size class), histograms)
+//   a3 bin / sort            k_scan_* + k_census<true> (counting sort of tet ids by tile and class) + k_items
 //   a4-a6 classify, clip, accumulate, flush    k_deposit_tiles (binned) / k_deposit_direct
 //   a7 patch path            the same kernels with Space::patch_mode = 1, k_patch_counts
 #pragma once
