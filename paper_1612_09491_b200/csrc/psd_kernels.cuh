@@ -537,7 +537,11 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     const int local = job - spre;
                     const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
                     const int nw = ((r16 >> 9) & 7) + 1;
-                    const int cv = (r16 & 7) + local / nw, cw = ((r16 >> 6) & 7) + local % nw;
+                    // local / nw for local < 64, nw <= 8 without an integer division:
+                    // (local * ceil(256 / nw)) >> 8 is exact there; the table holds ceil(256/nw) - 1
+                    const int inv = (int)((0x1f242a333f557fffull >> (8 * (nw - 1))) & 255ull) + 1;
+                    const int lq = (local * inv) >> 8;
+                    const int cv = (r16 & 7) + lq, cw = ((r16 >> 6) & 7) + (local - lq * nw);
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
                     // the face triangle, column-local, into slots 0..2 of the lane's polygon buffer
@@ -643,11 +647,19 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
 }
 
 // ---------------------------------------------------------------- direct path (any G)
-// One thread per tet, all its face jobs in sequence, polygon in local memory, global fp64
-// atomics with periodic wrap.  The plain path: PSD_OPT_KERNEL = 1, and grids the tiling does
-// not divide.
+// One thread per tet: all its face jobs (face, column) in ONE flattened loop (lanes of a warp run
+// the same job body whatever face or column they are at), polygon and tet-local vertices in
+// warp-interleaved shared memory, global fp64 reductions with periodic wrap.  The plain path:
+// PSD_OPT_KERNEL = 1, and grids the tiling does not divide.
+constexpr int DIR_THREADS = 128;
+constexpr int DIR_WARP_SCRATCH = (12 + 3 * POLY_CAP) * 32;  // doubles per warp
+
 template <bool COUNT>
-__global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
+__global__ void __launch_bounds__(DIR_THREADS) k_deposit_direct(DepositArgs A) {
+    __shared__ double scratch[(DIR_THREADS / 32) * DIR_WARP_SCRATCH];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* ts = scratch + warp * DIR_WARP_SCRATCH + lane;   // [12][32]: vertex v, coord x at (3v+x)*32
+    PolyBuf<32> poly{ts + 12 * 32};
     const int64_t ntet = (int64_t)6 * A.part.N * A.part.N * A.part.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     JobCounters cnt = {0, 0, 0, 0};
@@ -669,46 +681,74 @@ __global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
             }
         } else {
             const double w = A.weight_mode == 0 ? 6.0 * A.mass_per_tet / det : 1.0;
-            double polymem[3 * POLY_CAP];
-            PolyBuf<1> poly{polymem};
             int ax = A.chord_axis;
             if (ax < 0) {
                 int e0 = t.hi[0] - t.lo[0], e1 = t.hi[1] - t.lo[1], e2 = t.hi[2] - t.lo[2];
                 ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
             }
-            const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
-            // coordinates local to the tet's first cell (dynamic indexing: local memory, fine here)
-            double gl[4][3];
-            for (int v = 0; v < 4; ++v)
-                for (int x = 0; x < 3; ++x) gl[v][x] = t.g[v][x] - (double)t.lo[x];
-            const int nu = t.hi[ax] - t.lo[ax], nv = t.hi[av] - t.lo[av], nw = t.hi[aw] - t.lo[aw];
-#pragma unroll 1
+            const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
+            // coordinates local to the tet's first cell, in (u, v, w) order
+            int lo_u = 0, lo_v = 0, lo_w = 0, nu = 0, nv = 0, nw = 0;
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const int role = x == ax ? 0 : (x == av ? 1 : 2);
+                if (role == 0) { lo_u = t.lo[x]; nu = t.hi[x] - t.lo[x]; }
+                if (role == 1) { lo_v = t.lo[x]; nv = t.hi[x] - t.lo[x]; }
+                if (role == 2) { lo_w = t.lo[x]; nw = t.hi[x] - t.lo[x]; }
+#pragma unroll
+                for (int v = 0; v < 4; ++v) ts[(3 * v + role) * 32] = t.g[v][x] - (double)t.lo[x];
+            }
+            // per face: the rectangle of columns its projection meets (face f = vertices other than f)
+            int rv0[4], rv1[4], rw0[4], rw1[4];
+#pragma unroll
             for (int f = 0; f < 4; ++f) {
-                const unsigned int fv = FACE_TABLE >> (6 * f);
                 double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300;
+#pragma unroll
+                for (int v = 0; v < 4; ++v) {
+                    if (v == f) continue;
+                    const double cv = ts[(3 * v + 1) * 32], cw = ts[(3 * v + 2) * 32];
+                    mnv = fmin(mnv, cv); mxv = fmax(mxv, cv);
+                    mnw = fmin(mnw, cw); mxw = fmax(mxw, cw);
+                }
+                rv0[f] = max(__double2int_rd(mnv), 0); rv1[f] = min(__double2int_ru(mxv) - 1, nv);
+                rw0[f] = max(__double2int_rd(mnw), 0); rw1[f] = min(__double2int_ru(mxw) - 1, nw);
+                if (rv1[f] < rv0[f] || rw1[f] < rw0[f]) { rv1[f] = rv0[f] - 1; rw1[f] = rw0[f] - 1; }  // empty
+            }
+            // periodic wrap without a division per cell: the first cell wrapped once, then steps
+            const int wu0 = wrap_mod(lo_u, G), wv0 = wrap_mod(lo_v, G), ww0 = wrap_mod(lo_w, G);
+            auto wrapped = [G](int first, int off) { int c = first + off; while (c >= G) c -= G; return c; };
+            // strides of (u,v,w) in the grid, index (x*G+y)*G+z
+            const long long su = ax == 0 ? (long long)G * G : (ax == 1 ? G : 1);
+            const long long sv = av == 0 ? (long long)G * G : (av == 1 ? G : 1);
+            const long long sw = aw == 0 ? (long long)G * G : (aw == 1 ? G : 1);
+            // ---- the flattened job loop: state (f, cv, cw) advanced incrementally
+            int f = -1, cv = 0, cw = 0, v1 = -1, w0 = 0, w1 = -1;
+            for (;;) {
+                ++cw;
+                if (cw > w1) { cw = w0; ++cv; }
+                while (cv > v1) {  // next non-empty face
+                    ++f;
+                    if (f >= 4) break;
+                    const int a0 = f == 0 ? rv0[0] : (f == 1 ? rv0[1] : (f == 2 ? rv0[2] : rv0[3]));
+                    v1 = f == 0 ? rv1[0] : (f == 1 ? rv1[1] : (f == 2 ? rv1[2] : rv1[3]));
+                    w0 = f == 0 ? rw0[0] : (f == 1 ? rw0[1] : (f == 2 ? rw0[2] : rw0[3]));
+                    w1 = f == 0 ? rw1[0] : (f == 1 ? rw1[1] : (f == 2 ? rw1[2] : rw1[3]));
+                    cv = a0; cw = w0;
+                }
+                if (f >= 4) break;
+                const unsigned int fv = FACE_TABLE >> (6 * f);
+                const double ov = (double)cv, ow = (double)cw;
+#pragma unroll
                 for (int i = 0; i < 3; ++i) {
                     const int vi = (fv >> (2 * i)) & 3;
-                    mnv = fmin(mnv, gl[vi][av]); mxv = fmax(mxv, gl[vi][av]);
-                    mnw = fmin(mnw, gl[vi][aw]); mxw = fmax(mxw, gl[vi][aw]);
+                    poly.at(i, 0) = ts[(3 * vi + 0) * 32];
+                    poly.at(i, 1) = ts[(3 * vi + 1) * 32] - ov;
+                    poly.at(i, 2) = ts[(3 * vi + 2) * 32] - ow;
                 }
-                const int v0 = max(__double2int_rd(mnv), 0), v1 = min(__double2int_ru(mxv) - 1, nv);
-                const int w0 = max(__double2int_rd(mnw), 0), w1 = min(__double2int_ru(mxw) - 1, nw);
-                for (int cv = v0; cv <= v1; ++cv)
-                    for (int cw = w0; cw <= w1; ++cw) {
-                        for (int i = 0; i < 3; ++i) {
-                            const int vi = (fv >> (2 * i)) & 3;
-                            poly.at(i, 0) = gl[vi][ax];
-                            poly.at(i, 1) = gl[vi][av] - (double)cv;
-                            poly.at(i, 2) = gl[vi][aw] - (double)cw;
-                        }
-                        face_job<1, COUNT>(poly, 0, nu, [&](int c, double D) {
-                            int cc[3];
-                            cc[ax] = wrap_mod(t.lo[ax] + c, G);
-                            cc[av] = wrap_mod(t.lo[av] + cv, G);
-                            cc[aw] = wrap_mod(t.lo[aw] + cw, G);
-                            atomicAdd(&s.out[((long long)cc[0] * G + cc[1]) * G + cc[2]], w * D);
-                        }, &cnt);
-                    }
+                double* col = s.out + wrapped(wv0, cv) * sv + wrapped(ww0, cw) * sw;
+                face_job<32, COUNT>(poly, 0, nu, [&](int c, double D) {
+                    atomicAdd(col + wrapped(wu0, c) * su, w * D);
+                }, &cnt);
             }
         }
     }
@@ -724,23 +764,50 @@ __global__ void __launch_bounds__(128) k_deposit_direct(DepositArgs A) {
     }
 }
 
-// census-only statistics for the direct path (no tiles): sum/max cells, histogram, inverted
+// census-only statistics for the direct path (no tiles): sum/max cells, histogram, inverted.
+// Per-block partial results in shared memory, one set of global atomics per block.
 __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, unsigned long long* stats,
                                                    unsigned long long* hist) {
+    __shared__ unsigned int sh_hist[64];
+    __shared__ unsigned long long sh_stat[ST_COUNT];
+    if (threadIdx.x < 64) sh_hist[threadIdx.x] = 0;
+    if (threadIdx.x < ST_COUNT) sh_stat[threadIdx.x] = 0;
+    __syncthreads();
     int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (id >= ntet) return;
-    double P[4][3];
-    load_tet_vertices(p, id / 6, (int)(id % 6), P);
-    Tet t;
-    finish_tet(P, scale, t);
-    long long nc = (long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) * (t.hi[2] - t.lo[2] + 1);
-    atomicAdd(&stats[ST_SUM_CELLS], (unsigned long long)nc);
-    atomicMax(&stats[ST_MAX_CELLS], (unsigned long long)nc);
-    atomicAdd(&hist[bit_width_u64((unsigned long long)(nc - 1))], 1ull);
-    double det = tet_det(t.g);
-    if (det < 0.0) atomicAdd(&stats[ST_INVERTED], 1ull);
-    if (det == 0.0) atomicAdd(&stats[ST_DEGENERATE], 1ull);
+    unsigned long long nc = 0;
+    unsigned int inv = 0, deg = 0;
+    if (id < ntet) {
+        double P[4][3];
+        load_tet_vertices(p, id / 6, (int)(id % 6), P);
+        Tet t;
+        finish_tet(P, scale, t);
+        nc = (unsigned long long)((long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) * (t.hi[2] - t.lo[2] + 1));
+        atomicAdd(&sh_hist[bit_width_u64(nc - 1)], 1u);
+        double det = tet_det(t.g);
+        inv = det < 0.0; deg = det == 0.0;
+    }
+    // warp partials (64-bit sum and max by halves), then one shared atomic per warp
+    unsigned long long sum = nc, mx = nc;
+    for (int o = 16; o; o >>= 1) {
+        sum += __shfl_down_sync(0xffffffffu, sum, o);
+        unsigned long long y = __shfl_down_sync(0xffffffffu, mx, o);
+        mx = y > mx ? y : mx;
+    }
+    inv = __reduce_add_sync(0xffffffffu, inv);
+    deg = __reduce_add_sync(0xffffffffu, deg);
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&sh_stat[ST_SUM_CELLS], sum);
+        atomicMax(&sh_stat[ST_MAX_CELLS], mx);
+        if (inv) atomicAdd(&sh_stat[ST_INVERTED], (unsigned long long)inv);
+        if (deg) atomicAdd(&sh_stat[ST_DEGENERATE], (unsigned long long)deg);
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 && sh_hist[threadIdx.x]) atomicAdd(&hist[threadIdx.x], (unsigned long long)sh_hist[threadIdx.x]);
+    if (threadIdx.x == ST_SUM_CELLS && sh_stat[ST_SUM_CELLS]) atomicAdd(&stats[ST_SUM_CELLS], sh_stat[ST_SUM_CELLS]);
+    if (threadIdx.x == ST_MAX_CELLS) atomicMax(&stats[ST_MAX_CELLS], sh_stat[ST_MAX_CELLS]);
+    if (threadIdx.x == ST_INVERTED && sh_stat[ST_INVERTED]) atomicAdd(&stats[ST_INVERTED], sh_stat[ST_INVERTED]);
+    if (threadIdx.x == ST_DEGENERATE && sh_stat[ST_DEGENERATE]) atomicAdd(&stats[ST_DEGENERATE], sh_stat[ST_DEGENERATE]);
 }
 
 // ---------------------------------------------------------------- a7 refinement census
