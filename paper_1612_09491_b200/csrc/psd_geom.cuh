@@ -247,23 +247,18 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
     crossing_edges(mask, r.n, i_out, i_in);
     const int sa = slot_of(r.order, i_out ? i_out - 1 : r.n - 1), sb = slot_of(r.order, i_out);
     const int sc = slot_of(r.order, i_in ? i_in - 1 : r.n - 1), se = slot_of(r.order, i_in);
-    const double wallpos = up ? 1.0 : 0.0;
+    // signed distance to the wall: d = sgn * x + wallpos (inside: d >= 0)
+    const double sgn = up ? -1.0 : 1.0, wallpos = up ? 1.0 : 0.0;
+    const double da = fma(sgn, q.at(sa, ax), wallpos), db = fma(sgn, q.at(sb, ax), wallpos);
+    const double de = fma(sgn, q.at(se, ax), wallpos), dc = fma(sgn, q.at(sc, ax), wallpos);
+    const double t1 = da * fast_rcp(da - db);  // leaving crossing: inside a -> outside b
+    const double t2 = de * fast_rcp(de - dc);  // entering crossing: inside e -> outside c
     double xo[3], xi[3];
-    {   // leaving crossing: inside a -> outside b
-        const double a0 = q.at(sa, 0), a1 = q.at(sa, 1), a2 = q.at(sa, 2);
-        const double b0 = q.at(sb, 0), b1 = q.at(sb, 1), b2 = q.at(sb, 2);
-        const double ca = ax == 1 ? a1 : a2, cb = ax == 1 ? b1 : b2;
-        const double da = up ? 1.0 - ca : ca, db = up ? 1.0 - cb : cb;
-        const double t = da * fast_rcp(da - db);
-        xo[0] = fma(t, b0 - a0, a0); xo[1] = fma(t, b1 - a1, a1); xo[2] = fma(t, b2 - a2, a2);
-    }
-    {   // entering crossing: inside e -> outside c
-        const double e0 = q.at(se, 0), e1 = q.at(se, 1), e2 = q.at(se, 2);
-        const double c0 = q.at(sc, 0), c1 = q.at(sc, 1), c2 = q.at(sc, 2);
-        const double ce = ax == 1 ? e1 : e2, cc = ax == 1 ? c1 : c2;
-        const double de = up ? 1.0 - ce : ce, dc = up ? 1.0 - cc : cc;
-        const double t = de * fast_rcp(de - dc);
-        xi[0] = fma(t, c0 - e0, e0); xi[1] = fma(t, c1 - e1, e1); xi[2] = fma(t, c2 - e2, e2);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double a = q.at(sa, c), e = q.at(se, c);
+        xo[c] = fma(t1, q.at(sb, c) - a, a);
+        xi[c] = fma(t2, q.at(sc, c) - e, e);
     }
     if (ax == 1) { xo[1] = wallpos; xi[1] = wallpos; } else { xo[2] = wallpos; xi[2] = wallpos; }
     // new points go to the slots of the first and last removed vertex (already read); if only one
@@ -271,8 +266,8 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
     const int s_out = sb;
     int s_in = sc;
     if (sc == sb) s_in = r.fresh++;
-    q.at(s_out, 0) = xo[0]; q.at(s_out, 1) = xo[1]; q.at(s_out, 2) = xo[2];
-    q.at(s_in, 0) = xi[0]; q.at(s_in, 1) = xi[1]; q.at(s_in, 2) = xi[2];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { q.at(s_out, c) = xo[c]; q.at(s_in, c) = xi[c]; }
     // order: X_in, the inside run (starting at i_in), X_out
     const int m = __popc(mask);
     const unsigned rot = i_in ? ((r.order >> (4 * i_in)) | (r.order << (4 * (r.n - i_in)))) : r.order;
