@@ -409,29 +409,33 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
         if (lane == 0) base = atomicAdd(&sh_next, 32u);
         base = __shfl_sync(0xffffffffu, base, 0);
         if (base >= item.count) break;
-        // ---- a1: each lane builds one tet of the batch
+        // ---- a1: each lane builds one tet of the batch.  The tet is rebuilt from its id for every
+        // periodic image of the tile it meets (almost always one), so that nothing of stage A stays
+        // in registers across stages B and C.
         const bool have = base + lane < item.count;
-        Tet t;
-        double det = 1.0;
-        int nimg[3] = {1, 1, 1}, mlo[3] = {0, 0, 0};
-        if (have) {
-            unsigned int id = A.pair_ids[item.begin + base + lane];
-            double P[4][3];
-            load_tet_vertices(A.part, id / 6, id % 6, P);
-            finish_tet(P, scale, t);
-            det = tet_det(t.g);
-#pragma unroll
-            for (int x = 0; x < 3; ++x) {  // periodic images of this tile met by the tet's range
-                mlo[x] = -floor_div(org[x] + TILE - 1 - t.lo[x], Gl);
-                nimg[x] = floor_div(t.hi[x] - org[x], Gl) - mlo[x] + 1;
-            }
-        }
-        int my_images = have ? nimg[0] * nimg[1] * nimg[2] : 0;
-        const int max_images = __reduce_max_sync(0xffffffffu, my_images);
+        const unsigned int id = have ? A.pair_ids[item.begin + base + lane] : 0u;
+        int max_images = 1;
         for (int img = 0; img < max_images; ++img) {
             // ---- stage A: slot = lane.  Tile-local vertices, weight, face rectangles.
             unsigned int cnts = 0u;  // face jobs of this slot, 8 bits per face
             __syncwarp();
+            Tet t;
+            double det = 1.0;
+            int nimg[3] = {1, 1, 1}, mlo[3] = {0, 0, 0};
+            int my_images = 0;
+            if (have) {
+                double P[4][3];
+                load_tet_vertices(A.part, id / 6, id % 6, P);
+                finish_tet(P, scale, t);
+                det = tet_det(t.g);
+#pragma unroll
+                for (int x = 0; x < 3; ++x) {  // periodic images of this tile met by the tet's range
+                    mlo[x] = -floor_div(org[x] + TILE - 1 - t.lo[x], Gl);
+                    nimg[x] = floor_div(t.hi[x] - org[x], Gl) - mlo[x] + 1;
+                }
+                my_images = nimg[0] * nimg[1] * nimg[2];
+            }
+            if (img == 0) max_images = __reduce_max_sync(0xffffffffu, my_images);
             if (img < my_images) {
                 int m[3] = {mlo[0] + img % nimg[0], mlo[1] + (img / nimg[0]) % nimg[1],
                             mlo[2] + img / (nimg[0] * nimg[1])};
