@@ -472,6 +472,11 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         }
                         if (in) atomicAdd(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], A.mass_per_tet);
                     }
+                } else if (t.lo[0] == t.hi[0] && t.lo[1] == t.hi[1] && t.lo[2] == t.hi[2]) {
+                    // a4, tet inside one cell ("trivial cases"): the whole tet goes
+                    // to that cell -- m, or its signed volume det/6 in signed-volume mode
+                    atomicAdd(&acc[(lo[0] * TILE + lo[1]) * TILE + lo[2]],
+                              A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0));
                 } else {
 #pragma unroll
                     for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
@@ -683,6 +688,10 @@ __global__ void __launch_bounds__(DIR_THREADS) k_deposit_direct(DepositArgs A) {
                     c[x] = wrap_mod(__double2int_rd((t.g[0][x] + t.g[1][x] + t.g[2][x] + t.g[3][x]) / 4.0), G);
                 atomicAdd(&s.out[((long long)c[0] * G + c[1]) * G + c[2]], A.mass_per_tet);
             }
+        } else if (t.lo[0] == t.hi[0] && t.lo[1] == t.hi[1] && t.lo[2] == t.hi[2]) {
+            // a4, tet inside one cell: no clipping
+            atomicAdd(&s.out[((long long)wrap_mod(t.lo[0], G) * G + wrap_mod(t.lo[1], G)) * G + wrap_mod(t.lo[2], G)],
+                      A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0));
         } else {
             const double w = A.weight_mode == 0 ? 6.0 * A.mass_per_tet / det : 1.0;
             int ax = A.chord_axis;

@@ -34,6 +34,11 @@ CONFIGS = [
          stride=4, patches=dict(base_G=128, P=16, max_level=2, factor=4.0), same_particles_as=2),
     dict(name="cfg4_512_1024", N=512, G=1024, modes=256, kmax=32, rms=6.0, dtype="float32",
          stride=4),
+    # not in BASELINE.json: the paper's own analytic weak-scaling workload (PAPER.md:175,
+    # SURVEY.md 8(f) row 1): 512^3 particles on a lattice + independent uniform offsets of up to
+    # one lattice spacing per axis, deposited on 256^3 cells (G = N/2: most tets inside one cell)
+    dict(name="paper_weak_512_256", N=512, G=256, kind="jitter", amplitude=1.0, dtype="float32",
+         stride=4),
 ]
 
 
@@ -138,6 +143,9 @@ def zeldovich_positions(N: int, n_modes: int, kmax: int, rms_cells: float, seed:
 def config_positions(index: int, N_override: int | None = None):
     """Positions of BASELINE.json configs[index] (cfg3 uses cfg2's particles)."""
     cfg = CONFIGS[index]
+    if cfg.get("kind") == "jitter":
+        return jittered_lattice(N_override or cfg["N"], BASE_SEED + index, cfg["amplitude"],
+                                dtype=cfg["dtype"], stride=cfg["stride"])
     src = cfg.get("same_particles_as", index)
     c = CONFIGS[src]
     N = N_override or c["N"]
