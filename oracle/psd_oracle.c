@@ -30,6 +30,11 @@
  *   O5  counters compared bit-exactly with the GPU census (tile = 8^3 cells).
  *   O6  PAPER.md:72     patch deposit: same as O2-O4 on the level grid, restricted to
  *       the patch's P^3 box.   PAPER.md:66: refinement by tet count.
+ *   O7  PAPER.md:74-76  (section 4, Fig. 4) memory-lean refinement census: the Lagrangian
+ *       grid is cut into sub-blocks of B^3 cells, each sub-block's minimal axis-aligned
+ *       bounding box is taken, and the number of tets over a tree node is ESTIMATED as
+ *       (tets of the sub-block) x vol(box n node) / vol(box), summed over sub-blocks
+ *       (psdo_subblock_counts; reading Q17 for the fixed-point unit).
  *
  * Precision: REAL is double (the timed baseline) or __float128 ("gold", -DPSDO_GOLD)
  * for the geometry; sums into the output grid are always double.  The tet determinant
@@ -585,6 +590,82 @@ int psdo_patch_counts(const void *pos, int dtype, int stride, int N, double L, i
                 }
             }
     for (int x = 0; x < 3; ++x) free(seen[x]);
+    return 0;
+}
+
+/* O7.  counts[] is the dense (base_G/P * 2^level)^3 array of candidate patch
+ * positions; each receives, from every sub-block of B^3 Lagrangian cells (the last one per
+ * axis may be smaller), T_b * vol(AABB n patch) / vol(AABB) in units of 2^-20 tets, rounded
+ * to the nearest integer per (sub-block, patch) so that the sum does not depend on the order
+ * (T_b = 6 x cells of the sub-block; the AABB spans the sub-block's particles including the
+ * layer shared with the next sub-block, unwrapped to the minimum image of its first
+ * particle).  All arithmetic in double, one rounding per operation. */
+int psdo_subblock_counts(const void *pos, int dtype, int stride, int N, double L, int base_G, int P,
+                         int level, int B, uint64_t *counts) {
+    if (N < 2 || base_G % P || B < 1) return 1;
+    particles_t p = {pos, dtype, stride, N, L};
+    const int64_t G = (int64_t)base_G << level;
+    const int64_t np = G / P;
+    const double scale = (double)G / L;
+    const double Pc = (double)P;
+    memset(counts, 0, sizeof(uint64_t) * (size_t)(np * np * np));
+    const int nb = (N + B - 1) / B;
+    for (int bi = 0; bi < nb; ++bi)
+        for (int bj = 0; bj < nb; ++bj)
+            for (int bk = 0; bk < nb; ++bk) {
+                int o[3] = {bi * B, bj * B, bk * B}, n[3];
+                for (int x = 0; x < 3; ++x) n[x] = (o[x] + B <= N) ? B : N - o[x];
+                double ref[3], lo[3], hi[3];
+                int64_t ridx = ((int64_t)o[0] * N + o[1]) * N + o[2];
+                for (int c = 0; c < 3; ++c) lo[c] = hi[c] = ref[c] = (double)load_coord(&p, ridx, c);
+                for (int a = 0; a <= n[0]; ++a)
+                    for (int b = 0; b <= n[1]; ++b)
+                        for (int cc = 0; cc <= n[2]; ++cc) {
+                            int64_t idx = ((int64_t)((o[0] + a) % N) * N + (o[1] + b) % N) * N + (o[2] + cc) % N;
+                            for (int c = 0; c < 3; ++c) {
+                                double xv = (double)load_coord(&p, idx, c);
+                                double d = xv - ref[c];
+                                double q = d / L;
+                                double r = rint(q);
+                                double sft = L * r;
+                                xv = xv - sft;
+                                if (xv < lo[c]) lo[c] = xv;
+                                if (xv > hi[c]) hi[c] = xv;
+                            }
+                        }
+                const double Tfix = (double)(6 * (int64_t)n[0] * n[1] * n[2]) * 1048576.0;
+                int64_t first[3], cnt[3];
+                double frac[3][64];
+                int too_many = 0;
+                for (int x = 0; x < 3; ++x) {
+                    double glo = lo[x] * scale, ghi = hi[x] * scale;
+                    double ext = ghi - glo;
+                    first[x] = (int64_t)floor(glo / Pc);
+                    int64_t last = (int64_t)floor(ghi / Pc);
+                    cnt[x] = last - first[x] + 1;
+                    if (cnt[x] > 64) { too_many = 1; break; }
+                    for (int64_t q = 0; q < cnt[x]; ++q) {
+                        double a = (double)((first[x] + q) * P), b = (double)((first[x] + q + 1) * P);
+                        if (glo > a) a = glo;
+                        if (ghi < b) b = ghi;
+                        double ov = b - a;
+                        if (ov < 0.0) ov = 0.0;
+                        frac[x][q] = ext > 0.0 ? ov / ext : 1.0;
+                    }
+                }
+                if (too_many) return 2;
+                for (int64_t a = 0; a < cnt[0]; ++a)
+                    for (int64_t b = 0; b < cnt[1]; ++b)
+                        for (int64_t c = 0; c < cnt[2]; ++c) {
+                            double f = frac[0][a] * frac[1][b];
+                            f = f * frac[2][c];
+                            double e = Tfix * f;
+                            e = e + 0.5;
+                            uint64_t est = (uint64_t)floor(e);
+                            counts[(wrap(first[0] + a, np) * np + wrap(first[1] + b, np)) * np +
+                                   wrap(first[2] + c, np)] += est;
+                        }
+            }
     return 0;
 }
 

@@ -249,6 +249,26 @@ def patch_counts(pos, L, base_G: int, P: int, level: int) -> np.ndarray:
     return cnt
 
 
+SUBBLOCK_UNIT = 1 << 20  # subblock_counts are in units of 2^-20 tets
+
+
+def subblock_counts(pos, L, base_G: int, P: int, level: int, B: int = 8) -> np.ndarray:
+    """tets over each candidate patch position of `level`, ESTIMATED from the
+    bounding boxes of the B^3-cell Lagrangian sub-blocks (uint64, units of 2^-20 tets)."""
+    p, dt, stride, N = _pos_args(pos)
+    npos = (base_G << level) // P
+    cnt = np.zeros((npos, npos, npos), dtype=np.uint64)
+    lib = _lib()
+    lib.psdo_subblock_counts.restype = C.c_int
+    lib.psdo_subblock_counts.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int,
+                                         C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint64)]
+    rc = lib.psdo_subblock_counts(p, dt, stride, N, L, base_G, P, level, B,
+                                  cnt.ctypes.data_as(C.POINTER(C.c_uint64)))
+    if rc:
+        raise ValueError(f"psdo_subblock_counts: rc={rc}")
+    return cnt
+
+
 RULE_LITERAL_TOP_DOWN = 0
 RULE_BOTTOM_UP_LEVEL_MEAN = 1
 

@@ -183,3 +183,56 @@ def test_cfg0_has_no_shell_crossing(oracle):
     grid, st = oracle.deposit_uniform(pos, 1.0, 1.0, 64)
     assert st["n_tets"] == 196608 and st["n_inverted"] == 0
     assert abs(grid.sum() - 1.0) < 1e-12
+
+
+# ------------------------------------------------------------------ O7: sub-block AABB census
+def test_subblock_census_closed_form_on_the_aligned_lattice(oracle):
+    """PAPER.md:74-76.  Unperturbed lattice, N = 32, sub-blocks of 8^3 cells: every sub-block's
+    box is exactly its own Lagrangian cube, so a patch that IS a sub-block cube receives exactly
+    the sub-block's 6 x 8^3 tets, and a patch of half the edge exactly 1/8 of them."""
+    pos = psd_inputs.lattice(32)
+    unit = oracle.SUBBLOCK_UNIT
+    c = oracle.subblock_counts(pos, 1.0, 32, 8, 0)      # patch edge = sub-block edge
+    assert c.shape == (4, 4, 4) and np.all(c == 6 * 512 * unit)
+    c = oracle.subblock_counts(pos, 1.0, 32, 4, 0)      # 8 patches per sub-block
+    assert c.shape == (8, 8, 8) and np.all(c == 6 * 64 * unit)
+    c = oracle.subblock_counts(pos, 1.0, 32, 8, 1)      # level 1: the same patches in space
+    assert c.shape == (8, 8, 8) and np.all(c == 6 * 64 * unit)
+    c = oracle.subblock_counts(pos, 1.0, 32, 16, 0)     # 8 sub-blocks per patch
+    assert c.shape == (2, 2, 2) and np.all(c == 6 * 4096 * unit)
+
+
+@pytest.mark.parametrize("N,B,base_G,P,level", [(32, 8, 32, 8, 0), (32, 8, 32, 8, 1), (24, 8, 48, 4, 0),
+                                                (20, 8, 40, 8, 0), (32, 4, 16, 4, 1)])
+def test_subblock_census_conserves_the_tet_count(oracle, N, B, base_G, P, level):
+    """The shares of one box over the patches sum to 1, so the estimates sum to 6 N^3 -- up to the
+    half-unit rounding of each (sub-block, patch) term; also with a ragged last sub-block."""
+    pos = crossing_field(N, 1.5, seed=11, dtype="float32", stride=4)
+    c = oracle.subblock_counts(pos, 1.0, base_G, P, level, B)
+    total = int(c.sum(dtype=np.uint64))
+    assert abs(total - 6 * N ** 3 * oracle.SUBBLOCK_UNIT) <= 0.5 * 27 * 64 * ((N + B - 1) // B) ** 3
+
+
+def test_subblock_census_against_point_sampling(oracle):
+    """Brute force: uniform points in every sub-block's bounding box (boxes taken here with numpy
+    from the unwrapped particles), binned to patches, weighted with the sub-block's tet count."""
+    N, B, base_G, P = 32, 8, 32, 8
+    pos = crossing_field(N, 1.0, seed=5)
+    c = oracle.subblock_counts(pos, 1.0, base_G, P, 0, B).astype(np.float64) / oracle.SUBBLOCK_UNIT
+    rng = np.random.default_rng(3)
+    npatch = base_G // P
+    est = np.zeros((npatch,) * 3)
+    idx = np.arange(B + 1)
+    for bi in range(N // B):
+        for bj in range(N // B):
+            for bk in range(N // B):
+                sub = pos[np.ix_((bi * B + idx) % N, (bj * B + idx) % N, (bk * B + idx) % N)][..., :3]
+                ref = sub[0, 0, 0]
+                sub = sub - np.rint(sub - ref)          # minimum image of the first particle
+                lo, hi = sub.reshape(-1, 3).min(0), sub.reshape(-1, 3).max(0)
+                pts = lo + (hi - lo) * rng.random((4000, 3))
+                cell = np.floor(pts * npatch).astype(int) % npatch
+                np.add.at(est, (cell[:, 0], cell[:, 1], cell[:, 2]), 6 * B ** 3 / 4000.0)
+    # 64 boxes x 4000 points: per-patch sampling error ~ a few percent of the mean
+    assert np.abs(est - c).max() < 0.05 * c.mean()
+    assert abs(c.sum() - 6 * N ** 3) < 1e-3
