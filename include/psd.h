@@ -61,8 +61,19 @@ enum {
     PSD_OPT_COUNTERS = 2,    /* 1: also count face jobs / non-empty clips / plane integrals / cell
                                 shares written during deposits (slower; for the work model).    */
     PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 1024) */
-    PSD_OPT_CHORD_AXIS = 4   /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
+    PSD_OPT_CHORD_AXIS = 4,  /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
+    PSD_OPT_REFINE_SUBBLOCK = 5 /* census used by psd_refine_patches.  0 (default): every tet is
+                                counted.  B in 1..64: the paper's memory-lean
+                                estimate (B = 8 there): the Lagrangian grid is
+                                cut into sub-blocks of B^3 cells and a candidate patch receives
+                                6 B^3 x vol(box n patch) / vol(box) from each sub-block's
+                                bounding box; counts are then in units of 2^-20 tets
+                                (PSD_SUBBLOCK_UNIT).  Valid while every sub-block's box is
+                                shorter than L/2 (minimum-image unwrap) and meets at most 64
+                                patch positions per axis, else PSD_ERR_UNWRAP.                */
 };
+
+#define PSD_SUBBLOCK_UNIT (1u << 20)
 
 /* refinement rules (reading Q14 of PAPER.md:66) */
 enum { PSD_RULE_LITERAL_TOP_DOWN = 0, PSD_RULE_BOTTOM_UP_LEVEL_MEAN = 1 };
@@ -136,7 +147,8 @@ PSD_API int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accum
  *   out_host     receives the patches ordered by level then (ox,oy,oz); cap = its capacity
  *   n_out        number of patches (also when cap is too small: then PSD_ERR_INVALID_ARG)
  *   counts_host  optional: receives the dense count arrays of all levels, concatenated
- *                (sum over l of (base_G/P * 2^l)^3 uint64)
+ *                (sum over l of (base_G/P * 2^l)^3 uint64); tets, or 2^-20 tets when
+ *                PSD_OPT_REFINE_SUBBLOCK is set
  * Synchronous. */
 PSD_API int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
                        psd_patch* out_host, int64_t cap, int64_t* n_out, uint64_t* counts_host);

@@ -41,7 +41,7 @@ struct psd_ctx {
     Particles part{};
     bool built = false;
     double total_mass = 0.0;
-    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1;
+    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0;
     unsigned int chunk = 1024;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
         totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid;
@@ -372,19 +372,31 @@ int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double fa
         np[l] = (base_G << l) / P;
         off[l + 1] = off[l] + (long long)np[l] * np[l] * np[l];
     }
-    CK(ctx->refine_counts.ensure(sizeof(unsigned long long) * (size_t)off[nl]));
-    CK(cudaMemsetAsync(ctx->refine_counts.p, 0, sizeof(unsigned long long) * (size_t)off[nl], ctx->stream));
+    // one extra word at the end: boxes the sub-block census could not place
+    CK(ctx->refine_counts.ensure(sizeof(unsigned long long) * (size_t)(off[nl] + 1)));
+    CK(cudaMemsetAsync(ctx->refine_counts.p, 0, sizeof(unsigned long long) * (size_t)(off[nl] + 1), ctx->stream));
     const long long ntet = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
     for (int l = 0; l < nl; ++l) {
-        k_patch_counts<<<(unsigned int)((ntet + 255) / 256), 256, 0, ctx->stream>>>(
-            ctx->part, base_G, P, l, ctx->refine_counts.as<unsigned long long>() + off[l]);
+        unsigned long long* dst = ctx->refine_counts.as<unsigned long long>() + off[l];
+        if (ctx->refine_subblock > 0) {  // estimate from sub-block bounding boxes
+            const int B = ctx->refine_subblock;
+            const long long nb = (ctx->part.N + B - 1) / B;
+            k_subblock_counts<<<(unsigned int)((nb * nb * nb + 3) / 4), 128, 0, ctx->stream>>>(
+                ctx->part, base_G, P, l, B, dst,
+                reinterpret_cast<unsigned int*>(ctx->refine_counts.as<unsigned long long>() + off[nl]));
+        } else {  // every tet counted
+            k_patch_counts<<<(unsigned int)((ntet + 255) / 256), 256, 0, ctx->stream>>>(ctx->part, base_G, P, l, dst);
+        }
         ctx->launches += 1;
     }
     CK(cudaGetLastError());
-    std::vector<unsigned long long> cnt((size_t)off[nl]);
+    std::vector<unsigned long long> cnt((size_t)off[nl] + 1);
     CK(cudaMemcpyAsync(cnt.data(), ctx->refine_counts.p, sizeof(unsigned long long) * cnt.size(),
                        cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    if (cnt.back() != 0)
+        return fail(ctx, PSD_ERR_UNWRAP, "sub-block census: a bounding box spans more than 64 patch positions");
+    cnt.pop_back();
     if (counts_host) std::memcpy(counts_host, cnt.data(), sizeof(unsigned long long) * cnt.size());
 
     // ---- the rule, on integers (Q14)
@@ -545,6 +557,9 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
         case PSD_OPT_CHORD_AXIS:
             if (iv < -1 || iv > 2) return fail(ctx, PSD_ERR_INVALID_ARG, "chord axis must be -1..2");
             ctx->chord_axis = iv; return PSD_OK;
+        case PSD_OPT_REFINE_SUBBLOCK:
+            if (iv < 0 || iv > 64) return fail(ctx, PSD_ERR_INVALID_ARG, "sub-block edge must be 0 (off) or 1..64 cells");
+            ctx->refine_subblock = iv; return PSD_OK;
         default:
             return fail(ctx, PSD_ERR_INVALID_ARG, "unknown option key");
     }

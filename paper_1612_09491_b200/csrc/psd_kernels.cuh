@@ -846,4 +846,81 @@ __global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, i
     });
 }
 
+// a7: the memory-lean census.  One warp per sub-block of B^3 Lagrangian cells:
+// the lanes stride over its (B+1)^3 particles (unwrapped to the minimum image of the first one)
+// for the bounding box, then over the candidate patch positions the box meets; each receives
+// T_b * vol(box n patch) / vol(box) in units of 2^-20 tets, rounded per term so that the integer
+// sum is order independent (Q17).  Individually rounded IEEE operations throughout.
+__global__ void __launch_bounds__(128) k_subblock_counts(Particles p, int base_G, int P, int level, int B,
+                                                         unsigned long long* counts, unsigned int* overflow) {
+    const int N = p.N;
+    const int nb = (N + B - 1) / B;
+    const long long sb = blockIdx.x * 4ll + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (sb >= (long long)nb * nb * nb) return;
+    const int bk = (int)(sb % nb), bj = (int)((sb / nb) % nb), bi = (int)(sb / ((long long)nb * nb));
+    const int o[3] = {bi * B, bj * B, bk * B};
+    int n[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) n[x] = (o[x] + B <= N) ? B : N - o[x];
+    double ref[3], lo[3], hi[3];
+    load_pos(p, ((int64_t)o[0] * N + o[1]) * N + o[2], ref);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { lo[c] = ref[c]; hi[c] = ref[c]; }
+    const int n1 = n[1] + 1, n2 = n[2] + 1, npart = (n[0] + 1) * n1 * n2;
+    for (int q = lane; q < npart; q += 32) {
+        const int cc = q % n2, b = (q / n2) % n1, a = q / (n2 * n1);
+        int ii = o[0] + a, jj = o[1] + b, kk = o[2] + cc;
+        ii = ii >= N ? ii - N : ii; jj = jj >= N ? jj - N : jj; kk = kk >= N ? kk - N : kk;
+        double v[3];
+        load_pos(p, ((int64_t)ii * N + jj) * N + kk, v);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double x = unwrap1(v[c], ref[c], p.L);
+            lo[c] = fmin(lo[c], x); hi[c] = fmax(hi[c], x);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        for (int s = 16; s; s >>= 1) {
+            lo[c] = fmin(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], s));
+            hi[c] = fmax(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], s));
+        }
+    const int Gl = base_G << level;
+    const int np = Gl / P;
+    const double scale = __ddiv_rn((double)Gl, p.L), Pc = (double)P;
+    const double Tfix = (double)(6ll * n[0] * n[1] * n[2]) * 1048576.0;
+    double glo[3], ghi[3], ext[3];
+    int first[3], cnt[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        glo[x] = __dmul_rn(lo[x], scale); ghi[x] = __dmul_rn(hi[x], scale);
+        ext[x] = __dsub_rn(ghi[x], glo[x]);
+        first[x] = (int)floor(__ddiv_rn(glo[x], Pc));
+        cnt[x] = (int)floor(__ddiv_rn(ghi[x], Pc)) - first[x] + 1;
+    }
+    if (cnt[0] > 64 || cnt[1] > 64 || cnt[2] > 64) {  // the oracle refuses such a box too
+        if (lane == 0) atomicAdd(overflow, 1u);
+        return;
+    }
+    auto share = [&](int x, int q) {
+        double a = (double)((long long)(first[x] + q) * P), b = (double)((long long)(first[x] + q + 1) * P);
+        a = glo[x] > a ? glo[x] : a;
+        b = ghi[x] < b ? ghi[x] : b;
+        double ov = __dsub_rn(b, a);
+        ov = ov < 0.0 ? 0.0 : ov;
+        return ext[x] > 0.0 ? __ddiv_rn(ov, ext[x]) : 1.0;
+    };
+    const int total = cnt[0] * cnt[1] * cnt[2];
+    for (int q = lane; q < total; q += 32) {
+        const int c = q % cnt[2], b = (q / cnt[2]) % cnt[1], a = q / (cnt[2] * cnt[1]);
+        double f = __dmul_rn(share(0, a), share(1, b));
+        f = __dmul_rn(f, share(2, c));
+        const unsigned long long est = __double2ull_rd(__dadd_rn(__dmul_rn(Tfix, f), 0.5));
+        const long long key = ((long long)wrap_mod(first[0] + a, np) * np + wrap_mod(first[1] + b, np)) * np +
+                              wrap_mod(first[2] + c, np);
+        if (est) atomicAdd(&counts[key], est);
+    }
+}
+
 }  // namespace psd

@@ -230,6 +230,28 @@ def test_patches_parity_and_refinement(psd, ctx, oracle):
     assert_mass(mass[l0].sum())
 
 
+@pytest.mark.parametrize("N,B,dtype,stride", [(32, 8, "float32", 4), (40, 8, "float64", 3), (36, 8, "float32", 3),
+                                              (32, 4, "float32", 4)])
+def test_subblock_census_bit_exact_and_drives_the_refinement(psd, ctx, oracle, N, B, dtype, stride):
+    """a7 / PAPER.md:74-76: the sub-block bounding-box estimate (fixed point, order independent)
+    equals the oracle's on every level, with a ragged last sub-block (N = 36) too, and the patch
+    list the rule builds from it is the oracle's."""
+    pos = crossing_field(N, 1.5, dtype=dtype, stride=stride, modes=40, kmax=4)
+    base_G, P, max_level, factor = 32, 8, 2, 1.5
+    ctx.psd_build_tets(to_dev(pos))
+    ctx.psd_set_option(psd.OPT_REFINE_SUBBLOCK, B)
+    try:
+        patches, counts = ctx.psd_refine_patches(base_G, P, max_level, factor, want_counts=True)
+    finally:
+        ctx.psd_set_option(psd.OPT_REFINE_SUBBLOCK, 0)
+    ocounts = [oracle.subblock_counts(pos, 1.0, base_G, P, l, B) for l in range(max_level + 1)]
+    for a, b in zip(counts, ocounts):
+        assert np.array_equal(a, b)
+    assert psd.SUBBLOCK_UNIT == oracle.SUBBLOCK_UNIT
+    assert np.array_equal(patches, oracle.refine_patches(ocounts, factor))
+    assert (patches[:, 0] == 1).any()
+
+
 def test_patch_list_subset_and_order_independence(psd, ctx, oracle):
     pos = crossing_field(12, 2.0)
     patches = np.array([[1, 3, 0, 2], [0, 1, 1, 0], [2, 7, 7, 7], [0, 0, 0, 1], [1, 0, 3, 3]], dtype=np.int32)
