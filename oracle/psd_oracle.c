@@ -62,6 +62,15 @@ typedef __float128 DETREAL;
 #define R_FLOOR floorq
 #define R_RINT rintq
 #define R_FABS fabsq
+#elif defined(PSDO_SINGLE)
+/* the geometry (unwrap, scaling, splitting, leaf volumes) in fp32, determinant and sums in fp64:
+ * exists only to measure whether an fp32 clip could hold the parity tolerance (it does not;
+ * DESIGN.md section 4 item 4, tests/test_oracle_deposit.py) */
+typedef float REAL;
+typedef double DETREAL;
+#define R_FLOOR floorf
+#define R_RINT rintf
+#define R_FABS fabsf
 #else
 typedef double REAL;
 typedef long double DETREAL;

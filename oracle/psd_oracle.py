@@ -19,7 +19,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "psd_oracle.c")
 _LIBS = {"double": os.path.join(_HERE, "libpsd_oracle.so"),
-         "gold": os.path.join(_HERE, "libpsd_oracle_gold.so")}
+         "gold": os.path.join(_HERE, "libpsd_oracle_gold.so"),
+         "single": os.path.join(_HERE, "libpsd_oracle_single.so")}
 
 F32, F64 = 0, 1
 MODE_MASS, MODE_SIGNED = 0, 1
@@ -35,6 +36,8 @@ def build(force: bool = False) -> None:
                "-Wall", "-Wextra", _SRC, "-o", lib + ".tmp"]
         if kind == "gold":
             cmd += ["-DPSDO_GOLD", "-lquadmath"]
+        if kind == "single":
+            cmd += ["-DPSDO_SINGLE", "-Wno-maybe-uninitialized"]
         cmd += ["-lm"]
         subprocess.run(cmd, check=True)
         os.replace(lib + ".tmp", lib)

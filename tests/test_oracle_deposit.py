@@ -236,3 +236,19 @@ def test_subblock_census_against_point_sampling(oracle):
     # 64 boxes x 4000 points: per-patch sampling error ~ a few percent of the mean
     assert np.abs(est - c).max() < 0.05 * c.mean()
     assert abs(c.sum() - 6 * N ** 3) < 1e-3
+
+
+def test_fp32_geometry_does_not_hold_the_parity_tolerance(oracle):
+    """BASELINE north_star: "fp32 clip allowed only if it holds" |x - ref| <= 1e-9 max_cell +
+    1e-6 |ref| and total mass to 1e-10.  The oracle built with fp32 geometry (fp64 determinant and
+    sums) against the __float128 build on a crossing field: the double build sits ~1e-7 of the
+    tolerance away, the fp32 build exceeds it many times over -- which is why the CUDA path clips
+    in fp64 (DESIGN.md section 4 item 4)."""
+    pos = crossing_field(8, 2.0, dtype="float32", stride=4)
+    gold, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 16, kind="gold")
+    dbl, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 16, kind="double")
+    sgl, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 16, kind="single")
+    tol = 1e-9 * gold.max() + 1e-6 * np.abs(gold)
+    assert (np.abs(dbl - gold) / tol).max() < 1e-3
+    assert (np.abs(sgl - gold) / tol).max() > 5.0
+    assert abs(sgl.sum() - 1.0) > 1e-10 > abs(dbl.sum() - 1.0)
