@@ -71,6 +71,11 @@ enum {
                                 (PSD_SUBBLOCK_UNIT).  Valid while every sub-block's box is
                                 shorter than L/2 (minimum-image unwrap) and meets at most 64
                                 patch positions per axis, else PSD_ERR_UNWRAP.                */
+    ,
+    PSD_OPT_CLASS_SMALL_CELLS = 6 /* a3 size classes of the binned path: a (tet, tile) pair whose
+                                cell range covers at most this many cells of the tile is class
+                                "small", else "large"; a power of two in [1, 512] (default 8) so
+                                that the classes are unions of the census buckets hist_pair[b] */
 };
 
 #define PSD_SUBBLOCK_UNIT (1u << 20)

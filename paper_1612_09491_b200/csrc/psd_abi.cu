@@ -42,6 +42,7 @@ struct psd_ctx {
     bool built = false;
     double total_mass = 0.0;
     int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0;
+    long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 1024;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
         totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid;
@@ -82,6 +83,7 @@ int reset_stats(psd_ctx* ctx) {
 
 // census + scan + scatter + items + tile deposit over `n_tiles` tiles of `space`
 int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
+    space.class_small_max = ctx->class_small;
     cudaStream_t st = ctx->stream;
     const long long ncell = (long long)ctx->part.N * ctx->part.N * ctx->part.N;
     const long long n_bins = n_tiles * N_CLASSES;  // (tile, size class)
@@ -557,6 +559,10 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
         case PSD_OPT_CHORD_AXIS:
             if (iv < -1 || iv > 2) return fail(ctx, PSD_ERR_INVALID_ARG, "chord axis must be -1..2");
             ctx->chord_axis = iv; return PSD_OK;
+        case PSD_OPT_CLASS_SMALL_CELLS:
+            if (iv < 1 || iv > TILE_CELLS || (iv & (iv - 1)))
+                return fail(ctx, PSD_ERR_INVALID_ARG, "class threshold must be a power of two in [1, 512]");
+            ctx->class_small = iv; return PSD_OK;
         case PSD_OPT_REFINE_SUBBLOCK:
             if (iv < 0 || iv > 64) return fail(ctx, PSD_ERR_INVALID_ARG, "sub-block edge must be 0 (off) or 1..64 cells");
             ctx->refine_subblock = iv; return PSD_OK;

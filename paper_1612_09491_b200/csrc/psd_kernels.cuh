@@ -25,6 +25,7 @@ struct Space {
     long long lookup_off[8];  // start of each level in lookup
     double* out;
     double L;
+    long long class_small_max;  // a3: pairs covering at most this many cells of the tile are class "small"
 };
 
 __device__ __forceinline__ double level_scale(const Space& s, int level) {
@@ -40,7 +41,7 @@ struct Item { unsigned int tile; unsigned int count; unsigned long long begin; }
 // cell range covers <= 8 cells of the tile (buckets b <= 3 of the census histogram), class 1
 // "large" -- so the 32-pair batches a warp fetches hold tets of similar size.  Bin = tile * 2 + class.
 constexpr int N_CLASSES = 2;
-constexpr long long CLASS_SMALL_MAX_CELLS = 8;
+constexpr long long CLASS_SMALL_MAX_CELLS = 8;  // default of PSD_OPT_CLASS_SMALL_CELLS
 
 enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
        ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_COUNT };
@@ -169,7 +170,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                     long long id = tile_id_of(s, level, tx, ty, tz);
                     if (id < 0) return;
                     // size class of the pair: cells of the tet's range inside this tile (a3)
-                    const long long bin = id * N_CLASSES + (inside > CLASS_SMALL_MAX_CELLS ? 1 : 0);
+                    const long long bin = id * N_CLASSES + (inside > s.class_small_max ? 1 : 0);
                     if (!SCATTER) {
                         const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
                         if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&tile_counts[bin], (unsigned int)__popc(peers));

@@ -185,6 +185,19 @@ def test_census_bit_exact_with_images_and_inversions(psd, ctx, oracle):
         assert np.array_equal(cls.sum(axis=1), cen["tile_counts"].astype(np.int64))
         assert int(cls[:, 0].sum()) == int(cen["hist_pair"][:4].sum())
         assert int(cls[:, 1].sum()) == int(cen["hist_pair"][4:].sum())
+    # the class threshold is an option (a power of two: the classes stay unions of the buckets);
+    # the deposit does not depend on it
+    ref = ctx.psd_deposit_uniform(24).cpu().numpy()
+    for thr, nb in [(1, 1), (64, 7), (512, 10)]:
+        ctx.psd_set_option(psd.OPT_CLASS_SMALL_CELLS, thr)
+        g = ctx.psd_deposit_uniform(24).cpu().numpy()
+        cls = ctx.psd_get_tile_class_counts().astype(np.int64)
+        cen = oracle.census(pos, 1.0, 24)
+        assert int(cls[:, 0].sum()) == int(cen["hist_pair"][:nb].sum())
+        assert np.allclose(g, ref, rtol=1e-9, atol=1e-18)
+    ctx.psd_set_option(psd.OPT_CLASS_SMALL_CELLS, 8)
+    with pytest.raises(psd.PsdError):
+        ctx.psd_set_option(psd.OPT_CLASS_SMALL_CELLS, 12)
 
 
 @pytest.mark.parametrize("chunk", [32, 100, 1024])
