@@ -291,7 +291,11 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
 template <int S>
 __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, int n, double a) {
     unsigned mask = 0;
-    for (int i = 0; i < n; ++i) mask |= (unsigned)(q.at(slot_of(order, i), 0) >= a) << i;
+#pragma unroll
+    for (int i = 0; i < POLY_CAP - 1; ++i) {
+        if (i >= n) break;
+        mask |= (unsigned)(q.at(slot_of(order, i), 0) >= a) << i;
+    }
     const unsigned full = (1u << n) - 1u;
     if (mask == 0 || mask == full) return 0.0;  // not a cutting plane (caller excludes this)
     int i_out, i_in;
@@ -317,7 +321,9 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
         pv = ev - x0v; pw = ew - x0w; ph = he;
     }
     double sum = 0.0;
-    for (int j = 1; j <= m; ++j) {
+#pragma unroll
+    for (int j = 1; j < POLY_CAP - 1; ++j) {
+        if (j > m) break;
         double cv, cw, ch;
         if (j < m) {
             const int s = (rot >> (4 * j)) & 7;
@@ -377,7 +383,9 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
     double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
     double umin = fmin(u0, lu), umax = fmax(u0, lu), A2 = 0.0, M6 = 0.0;
-    for (int i = 2; i < r.n; ++i) {
+#pragma unroll
+    for (int i = 2; i < POLY_CAP - 1; ++i) {
+        if (i >= r.n) break;
         const int s = slot_of(r.order, i);
         const double cu = q.at(s, 0), cv = q.at(s, 1) - v0, cw = q.at(s, 2) - w0;
         const double cr = lv * cw - lw * cv;
