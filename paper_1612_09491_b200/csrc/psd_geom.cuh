@@ -322,18 +322,14 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
     }
     double sum = 0.0;
 #pragma unroll
-    for (int j = 1; j < POLY_CAP - 1; ++j) {
-        if (j > m) break;
-        double cv, cw, ch;
-        if (j < m) {
-            const int s = (rot >> (4 * j)) & 7;
-            cv = q.at(s, 1) - x0v; cw = q.at(s, 2) - x0w; ch = q.at(s, 0) - a;
-        } else {
-            cv = xov - x0v; cw = xow - x0w; ch = 0.0;
-        }
+    for (int j = 1; j < POLY_CAP - 1; ++j) {  // the inside vertices after the first
+        if (j >= m) break;
+        const int s = (rot >> (4 * j)) & 7;
+        const double cv = q.at(s, 1) - x0v, cw = q.at(s, 2) - x0w, ch = q.at(s, 0) - a;
         sum = fma(pv * cw - pw * cv, ph + ch, sum);
         pv = cv; pw = cw; ph = ch;
     }
+    sum = fma(pv * (xow - x0w) - pw * (xov - x0v), ph, sum);  // last triangle: up to X_out (height 0)
     return sum;
 }
 
@@ -356,7 +352,7 @@ struct FaceClip {
 
 // q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
 // corner (the column is the unit square [0,1]^2).
-template <int S>
+template <int S, bool WALLS_UNROLLED = false>
 __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     FaceClip fc;
     fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.umin = fc.umax = 0.0;
@@ -372,10 +368,18 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     if (any_in != 15u) return fc;  // all three vertices outside one wall
     PolyRef r{0x210u, oc, 3, 3};
     unsigned pending = all_in ^ 15u;
-    while (pending && r.n) {
-        const int wall = __ffs(pending) - 1;
-        pending &= pending - 1;
-        clip_wall<S>(q, r, wall);
+    if (WALLS_UNROLLED) {
+        // the 4 walls in turn with a compile-time wall id (axis, side and outcode bit folded):
+        // pays in the thread-per-tet kernel, not in the tile kernel (code size, registers)
+#pragma unroll
+        for (int wall = 0; wall < 4; ++wall)
+            if (((pending >> wall) & 1u) && r.n) clip_wall<S>(q, r, wall);
+    } else {
+        while (pending && r.n) {
+            const int wall = __ffs(pending) - 1;
+            pending &= pending - 1;
+            clip_wall<S>(q, r, wall);
+        }
     }
     if (r.n < 3) return fc;
     // signed projected area A and first moment M1 = integral of u over Q, fan from vertex 0
@@ -427,7 +431,7 @@ __device__ __forceinline__ FaceRun face_run(const FaceClip& fc, int c_lo, int c_
 template <int S, bool COUNT, class Emit>
 __device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit emit, JobCounters* cnt) {
     if (COUNT) cnt->jobs++;
-    const FaceClip fc = face_clip<S>(q);
+    const FaceClip fc = face_clip<S, true>(q);
     const FaceRun fr = face_run(fc, c_lo, c_hi);
     if (fc.n < 3 || fc.umax <= (double)c_lo) return;
     if (COUNT) cnt->face_clips++;

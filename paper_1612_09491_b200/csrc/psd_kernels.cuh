@@ -479,30 +479,33 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     atomicAdd(&acc[(lo[0] * TILE + lo[1]) * TILE + lo[2]],
                               A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0));
                 } else {
+                    // per vertex: floor / ceil of (v, w) and ceil of u, read back through the
+                    // runtime axis (the lane's own stores above); the faces' rectangles are then
+                    // integer min / max (floor and ceil are monotone)
+                    int fv[4], cvv[4], fw[4], cww[4], cuu[4];
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) {
+                        const double pu = wtet[(3 * v + ax) * 32 + lane], pv = wtet[(3 * v + av) * 32 + lane];
+                        const double pw = wtet[(3 * v + aw) * 32 + lane];
+                        fv[v] = __double2int_rd(pv); cvv[v] = __double2int_ru(pv);
+                        fw[v] = __double2int_rd(pw); cww[v] = __double2int_ru(pw);
+                        cuu[v] = __double2int_ru(pu);
+                    }
+                    const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
+                    const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
+                    const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
+                    const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
+                    const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
 #pragma unroll
                     for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
-                        double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300, mxu = -1e300;
-#pragma unroll
-                        for (int v = 0; v < 4; ++v) {
-                            if (v == f) continue;
-                            // av, aw, ax are runtime: select instead of indexing
-                            double cu = ax == 0 ? gl[v][0] : (ax == 1 ? gl[v][1] : gl[v][2]);
-                            double cv = av == 0 ? gl[v][0] : (av == 1 ? gl[v][1] : gl[v][2]);
-                            double cw = aw == 0 ? gl[v][0] : (aw == 1 ? gl[v][1] : gl[v][2]);
-                            mnv = fmin(mnv, cv); mxv = fmax(mxv, cv);
-                            mnw = fmin(mnw, cw); mxw = fmax(mxw, cw);
-                            mxu = fmax(mxu, cu);
-                        }
-                        const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
-                        const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
-                        const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
-                        const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
-                        const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                        const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;
                         // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
-                        const int v0 = max(__double2int_rd(mnv), lov), v1 = min(__double2int_ru(mxv) - 1, hiv);
-                        const int w0 = max(__double2int_rd(mnw), low), w1 = min(__double2int_ru(mxw) - 1, hiw);
+                        const int v0 = max(min(min(fv[a], fv[b]), fv[d]), lov);
+                        const int v1 = min(max(max(cvv[a], cvv[b]), cvv[d]) - 1, hiv);
+                        const int w0 = max(min(min(fw[a], fw[b]), fw[d]), low);
+                        const int w1 = min(max(max(cww[a], cww[b]), cww[d]) - 1, hiw);
                         int c = 0;
-                        if (v1 >= v0 && w1 >= w0 && mxu > (double)lou) {
+                        if (v1 >= v0 && w1 >= w0 && max(max(cuu[a], cuu[b]), cuu[d]) > lou) {
                             c = (v1 - v0 + 1) * (w1 - w0 + 1);
                             rect |= (unsigned long long)(v0 | (v1 - v0) << 3 | w0 << 6 | (w1 - w0) << 9) << (16 * f);
                         }
@@ -578,7 +581,10 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         const int colofs = cv * sv + cw * sw;
                         // trivial part: cells entirely below Q get its projected area, the cell
                         // holding umin gets M1 - c A
-                        for (int c = c_lo; c <= fr.t_hi; ++c) {
+#pragma unroll
+                        for (int cc = 0; cc < TILE; ++cc) {
+                            const int c = c_lo + cc;
+                            if (c > fr.t_hi) break;
                             const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
                             if (D != 0.0) {
                                 atomicAdd(acc + colofs + c * su, f_w * D);
