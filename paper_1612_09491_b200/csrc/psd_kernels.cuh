@@ -71,6 +71,24 @@ __device__ __forceinline__ void for_each_block(const int lo[3], const int hi[3],
         b0[x] = floor_div(lo[x], bs);
         cnt[x] = min(floor_div(hi[x], bs) - b0[x] + 1, nb);
     }
+    // common case: the range is short enough on every axis to meet each block in one periodic
+    // image only -> no division, the per-axis terms hoisted out of the inner loops
+    if (hi[0] - lo[0] < Gl - bs && hi[1] - lo[1] < Gl - bs && hi[2] - lo[2] < Gl - bs) {
+        auto wrap1 = [nb](int v) {
+            int r = v < 0 ? v + nb : (v >= nb ? v - nb : v);
+            return (unsigned)r < (unsigned)nb ? r : wrap_mod(v, nb);
+        };
+        auto cells = [bs](int l, int h, int b) { return min(h, b * bs + bs - 1) - max(l, b * bs) + 1; };
+        for (int qx = 0; qx < cnt[0]; ++qx) {
+            const int bx = wrap1(b0[0] + qx), cx = cells(lo[0], hi[0], b0[0] + qx);
+            for (int qy = 0; qy < cnt[1]; ++qy) {
+                const int by = wrap1(b0[1] + qy), cxy = cx * cells(lo[1], hi[1], b0[1] + qy);
+                for (int qz = 0; qz < cnt[2]; ++qz)
+                    f(bx, by, wrap1(b0[2] + qz), (long long)cxy * cells(lo[2], hi[2], b0[2] + qz));
+            }
+        }
+        return;
+    }
     for (int qx = 0; qx < cnt[0]; ++qx)
         for (int qy = 0; qy < cnt[1]; ++qy)
             for (int qz = 0; qz < cnt[2]; ++qz) {
@@ -720,19 +738,21 @@ __global__ void __launch_bounds__(DIR_THREADS) k_deposit_direct(DepositArgs A) {
             }
             // per face: the rectangle of columns its projection meets (face f = vertices other than f)
             int rv0[4], rv1[4], rw0[4], rw1[4];
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-                double mnv = 1e300, mxv = -1e300, mnw = 1e300, mxw = -1e300;
+            {
+                int fv[4], cvv[4], fw[4], cww[4];  // per-vertex floors / ceils; integer min / max per face
 #pragma unroll
                 for (int v = 0; v < 4; ++v) {
-                    if (v == f) continue;
                     const double cv = ts[(3 * v + 1) * 32], cw = ts[(3 * v + 2) * 32];
-                    mnv = fmin(mnv, cv); mxv = fmax(mxv, cv);
-                    mnw = fmin(mnw, cw); mxw = fmax(mxw, cw);
+                    fv[v] = __double2int_rd(cv); cvv[v] = __double2int_ru(cv);
+                    fw[v] = __double2int_rd(cw); cww[v] = __double2int_ru(cw);
                 }
-                rv0[f] = max(__double2int_rd(mnv), 0); rv1[f] = min(__double2int_ru(mxv) - 1, nv);
-                rw0[f] = max(__double2int_rd(mnw), 0); rw1[f] = min(__double2int_ru(mxw) - 1, nw);
-                if (rv1[f] < rv0[f] || rw1[f] < rw0[f]) { rv1[f] = rv0[f] - 1; rw1[f] = rw0[f] - 1; }  // empty
+#pragma unroll
+                for (int f = 0; f < 4; ++f) {
+                    const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;
+                    rv0[f] = max(min(min(fv[a], fv[b]), fv[d]), 0); rv1[f] = min(max(max(cvv[a], cvv[b]), cvv[d]) - 1, nv);
+                    rw0[f] = max(min(min(fw[a], fw[b]), fw[d]), 0); rw1[f] = min(max(max(cww[a], cww[b]), cww[d]) - 1, nw);
+                    if (rv1[f] < rv0[f] || rw1[f] < rw0[f]) { rv1[f] = rv0[f] - 1; rw1[f] = rw0[f] - 1; }  // empty
+                }
             }
             // periodic wrap without a division per cell: the first cell wrapped once, then steps
             const int wu0 = wrap_mod(lo_u, G), wv0 = wrap_mod(lo_v, G), ww0 = wrap_mod(lo_w, G);
