@@ -347,7 +347,7 @@ struct FaceClip {
     unsigned order;
     int n;            // 0: empty
     double A, M1;     // signed projected area of Q, first moment integral of u over Q
-    double umin, umax;
+    int ifl, ice;     // floor of the lowest, ceil of the highest vertex height
 };
 
 // q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
@@ -355,7 +355,7 @@ struct FaceClip {
 template <int S, bool WALLS_UNROLLED = false>
 __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     FaceClip fc;
-    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.umin = fc.umax = 0.0;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
     unsigned oc = 0, all_in = 15u, any_in = 0u;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
@@ -386,7 +386,8 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     const int s0 = slot_of(r.order, 0), s1 = slot_of(r.order, 1);
     const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
     double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
-    double umin = fmin(u0, lu), umax = fmax(u0, lu), A2 = 0.0, M6 = 0.0;
+    int ifl = min(__double2int_rd(u0), __double2int_rd(lu)), ice = max(__double2int_ru(u0), __double2int_ru(lu));
+    double A2 = 0.0, M6 = 0.0;
 #pragma unroll
     for (int i = 2; i < POLY_CAP - 1; ++i) {
         if (i >= r.n) break;
@@ -395,12 +396,12 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
         const double cr = lv * cw - lw * cv;
         A2 += cr;
         M6 = fma(cr, u0 + lu + cu, M6);
-        umin = fmin(umin, cu); umax = fmax(umax, cu);
+        ifl = min(ifl, __double2int_rd(cu)); ice = max(ice, __double2int_ru(cu));
         lu = cu; lv = cv; lw = cw;
     }
     fc.order = r.order; fc.n = r.n;
     fc.A = 0.5 * A2; fc.M1 = M6 * (1.0 / 6.0);
-    fc.umin = umin; fc.umax = umax;
+    fc.ifl = ifl; fc.ice = ice;
     return fc;
 }
 
@@ -417,9 +418,8 @@ struct FaceRun {
 __device__ __forceinline__ FaceRun face_run(const FaceClip& fc, int c_lo, int c_hi) {
     FaceRun fr;
     fr.t_hi = c_lo - 1; fr.a_first = 0; fr.a_last = -1;
-    if (fc.n < 3 || fc.umax <= (double)c_lo) return fr;
-    const int fl = fc.umin >= (double)(c_hi + 1) ? c_hi + 1 : __double2int_rd(fc.umin);  // clamp before converting
-    const int ce = fc.umax >= (double)(c_hi + 2) ? c_hi + 2 : __double2int_ru(fc.umax);
+    if (fc.n < 3 || fc.ice <= c_lo) return fr;
+    const int fl = min(fc.ifl, c_hi + 1), ce = min(fc.ice, c_hi + 2);
     const int top = min(c_hi, ce - 1);
     fr.t_hi = min(top, fl);
     fr.a_first = max(c_lo, fl + 1);
@@ -433,10 +433,10 @@ __device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit 
     if (COUNT) cnt->jobs++;
     const FaceClip fc = face_clip<S, true>(q);
     const FaceRun fr = face_run(fc, c_lo, c_hi);
-    if (fc.n < 3 || fc.umax <= (double)c_lo) return;
+    if (fc.n < 3 || fc.ice <= c_lo) return;
     if (COUNT) cnt->face_clips++;
     for (int c = c_lo; c <= fr.t_hi; ++c) {
-        const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
+        const double D = c + 1 <= fc.ifl ? fc.A : fma(-(double)c, fc.A, fc.M1);
         if (D != 0.0) { emit(c, D); if (COUNT) cnt->cells++; }
     }
     for (int a = fr.a_first; a <= fr.a_last; ++a) {

@@ -357,7 +357,7 @@ struct DepositArgs {
 };
 
 #ifndef DEP_MIN_CTAS
-#define DEP_MIN_CTAS 4
+#define DEP_MIN_CTAS 5
 #endif
 #ifndef DEP_WARPS_N
 #define DEP_WARPS_N 4
@@ -589,7 +589,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     f_w = ts[12 * 32];
                     if (COUNT) cnt.jobs++;
                     const FaceClip fc = face_clip<32>(poly);
-                    if (fc.n >= 3 && fc.umax > (double)c_lo) {
+                    if (fc.n >= 3 && fc.ice > c_lo) {
                         if (COUNT) cnt.face_clips++;
                         const FaceRun fr = face_run(fc, c_lo, c_hi);
                         // strides of (u,v,w) in the 8^3 accumulator, index (x*8+y)*8+z
@@ -603,7 +603,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         for (int cc = 0; cc < TILE; ++cc) {
                             const int c = c_lo + cc;
                             if (c > fr.t_hi) break;
-                            const double D = (double)(c + 1) <= fc.umin ? fc.A : fma(-(double)c, fc.A, fc.M1);
+                            const double D = c + 1 <= fc.ifl ? fc.A : fma(-(double)c, fc.A, fc.M1);
                             if (D != 0.0) {
                                 atomicAdd(acc + colofs + c * su, f_w * D);
                                 if (COUNT) cnt.cells++;
