@@ -234,8 +234,8 @@ __device__ __forceinline__ void crossing_edges(unsigned mask, int n, int& i_out,
 // Clip the polygon against one wall of the column: wall 0: v >= 0, 1: v <= 1, 2: w >= 0,
 // 3: w <= 1 (a runtime value, so lanes clipping different walls run the same instructions).
 // Vertices exactly on the wall are inside; a convex polygon crosses the wall on exactly two edges,
-// each crossing is interpolated from its inside endpoint (ratio in [0,1]) and put exactly on the wall.
-template <int S>
+// each crossing is interpolated from its inside endpoint (ratio in [0,1]) and, with SNAP, put exactly on the wall.
+template <int S, bool SNAP>
 __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
     const int ax = 1 + (wall >> 1);
     const bool up = wall & 1;
@@ -260,7 +260,10 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
         xo[c] = fma(t1, q.at(sb, c) - a, a);
         xi[c] = fma(t2, q.at(sc, c) - e, e);
     }
-    if (ax == 1) { xo[1] = wallpos; xi[1] = wallpos; } else { xo[2] = wallpos; xi[2] = wallpos; }
+    // put the new points exactly on the wall where that is free (compile-time wall id); with a
+    // runtime wall id it costs 8 selects and changes nothing: the new points' outcodes for this
+    // wall are set, not computed, and an offset of one rounding error is below the clip's own
+    if (SNAP) { if (ax == 1) { xo[1] = wallpos; xi[1] = wallpos; } else { xo[2] = wallpos; xi[2] = wallpos; } }
     // new points go to the slots of the first and last removed vertex (already read); if only one
     // vertex was removed the second point takes a fresh slot
     const int s_out = sb;
@@ -373,12 +376,12 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
         // pays in the thread-per-tet kernel, not in the tile kernel (code size, registers)
 #pragma unroll
         for (int wall = 0; wall < 4; ++wall)
-            if (((pending >> wall) & 1u) && r.n) clip_wall<S>(q, r, wall);
+            if (((pending >> wall) & 1u) && r.n) clip_wall<S, true>(q, r, wall);
     } else {
         while (pending && r.n) {
             const int wall = __ffs(pending) - 1;
             pending &= pending - 1;
-            clip_wall<S>(q, r, wall);
+            clip_wall<S, false>(q, r, wall);
         }
     }
     if (r.n < 3) return fc;
