@@ -30,7 +30,7 @@ namespace psd {
 
 constexpr int TILE = 8;            // tile edge in cells (BASELINE north_star: 8^3-cell tiles)
 constexpr int TILE_CELLS = 512;
-constexpr int POLY_CAP = 8;        // triangle + 4 column planes -> <= 7 vertices
+constexpr int POLY_CAP = 7;        // triangle + 4 column planes -> <= 7 vertices, slots 0..6
 
 // Kuhn / Freudenthal split: every tet is (corner 0, a, b, corner 7); corner index
 // bit0 = +x, bit1 = +y, bit2 = +z.  Own copy (the oracle has its own).
@@ -202,7 +202,7 @@ struct PolyBuf {
 // A convex polygon as a CYCLIC ORDER over storage slots: nibble i of `order` is the slot (0..6)
 // holding vertex i; vertices never move, a clip only writes its two new points and re-packs the
 // order word.  Slots 0..2 hold the face triangle; each clip allocates at most one fresh slot
-// (`fresh`), so 3 + 4 walls = 7 slots suffice (POLY_CAP = 8).
+// (`fresh`), so 3 + 4 walls = 7 slots suffice (POLY_CAP).
 struct PolyRef {
     unsigned order;
     unsigned oc;  // nibble i = outcode of vertex i: bit k set = inside wall k (0: v>=0, 1: v<=1, 2: w>=0, 3: w<=1)
@@ -295,7 +295,7 @@ template <int S>
 __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, int n, double a) {
     unsigned mask = 0;
 #pragma unroll
-    for (int i = 0; i < POLY_CAP - 1; ++i) {
+    for (int i = 0; i < POLY_CAP; ++i) {
         if (i >= n) break;
         mask |= (unsigned)(q.at(slot_of(order, i), 0) >= a) << i;
     }
@@ -325,7 +325,7 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
     }
     double sum = 0.0;
 #pragma unroll
-    for (int j = 1; j < POLY_CAP - 1; ++j) {  // the inside vertices after the first
+    for (int j = 1; j < POLY_CAP; ++j) {  // the inside vertices after the first
         if (j >= m) break;
         const int s = (rot >> (4 * j)) & 7;
         const double cv = q.at(s, 1) - x0v, cw = q.at(s, 2) - x0w, ch = q.at(s, 0) - a;
@@ -355,11 +355,11 @@ struct FaceClip {
 
 // q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
 // corner (the column is the unit square [0,1]^2).
-template <int S, bool WALLS_UNROLLED = false>
-__device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
-    FaceClip fc;
-    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
-    unsigned oc = 0, all_in = 15u, any_in = 0u;
+// outcodes of the triangle in slots 0..2 (nibble i = vertex i, see PolyRef::oc), their AND and OR
+template <int S>
+__device__ __forceinline__ unsigned tri_outcodes(PolyBuf<S> q, unsigned& all_in, unsigned& any_in) {
+    unsigned oc = 0;
+    all_in = 15u; any_in = 0u;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const double v = q.at(i, 1), w = q.at(i, 2);
@@ -368,6 +368,24 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
         oc |= o << (4 * i);
         all_in &= o; any_in |= o;
     }
+    return oc;
+}
+
+template <int S, bool WALLS_UNROLLED>
+__device__ __forceinline__ FaceClip face_clip_oc(PolyBuf<S> q, unsigned oc, unsigned all_in, unsigned any_in);
+
+template <int S, bool WALLS_UNROLLED = false>
+__device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
+    unsigned all_in, any_in;
+    const unsigned oc = tri_outcodes<S>(q, all_in, any_in);
+    return face_clip_oc<S, WALLS_UNROLLED>(q, oc, all_in, any_in);
+}
+
+// the clip proper, outcodes given (the pooled tile kernel computes them when it sorts the jobs)
+template <int S, bool WALLS_UNROLLED>
+__device__ __forceinline__ FaceClip face_clip_oc(PolyBuf<S> q, unsigned oc, unsigned all_in, unsigned any_in) {
+    FaceClip fc;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
     if (any_in != 15u) return fc;  // all three vertices outside one wall
     PolyRef r{0x210u, oc, 3, 3};
     unsigned pending = all_in ^ 15u;
@@ -392,7 +410,7 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
     int ifl = min(__double2int_rd(u0), __double2int_rd(lu)), ice = max(__double2int_ru(u0), __double2int_ru(lu));
     double A2 = 0.0, M6 = 0.0;
 #pragma unroll
-    for (int i = 2; i < POLY_CAP - 1; ++i) {
+    for (int i = 2; i < POLY_CAP; ++i) {
         if (i >= r.n) break;
         const int s = slot_of(r.order, i);
         const double cu = q.at(s, 0), cv = q.at(s, 1) - v0, cw = q.at(s, 2) - w0;

@@ -365,8 +365,9 @@ struct DepositArgs {
 constexpr int DEP_WARPS = DEP_WARPS_N;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
-// [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32)
-constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP) * 32 + 32 + 16;
+// [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32), job queues (u32)
+constexpr int N_QUEUES = 3, QUEUE_CAP = 64;  // job queues by clip class, u32 descriptors
+constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP) * 32 + 32 + 16 + N_QUEUES * QUEUE_CAP / 2;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
 
 __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile, int& level,
@@ -394,8 +395,11 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
 //   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
 //            into the warp's slots; per face the rectangle of columns its projection meets.
 //   stage B  the face jobs (slot, face, column) of the 32 slots are numbered by a warp prefix
-//            sum of the rectangle sizes; lane = job, 32 jobs at a time, every lane busy.
-//   stage C  face_job: wall clip, closed-form plane integrals, shares added to the tile (a4-a6).
+//            sum of the rectangle sizes; lane = job computes its triangle's outcodes and queues
+//            the job by clip class (how many walls have a vertex beyond them).
+//   stage C  32 jobs of one queue at a time, lane = job: wall clip, trivial cells; then the
+//            cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
+//            integrals, shares added to the tile (a4-a6).
 // The tile is flushed to global memory with fp64 reductions at the end (a6).
 template <bool COUNT>
 __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
@@ -406,6 +410,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
     double* wpoly = wtet + 13 * 32;                                                    // [24][32]
     unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * POLY_CAP * 32);  // [32]
     unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 32);                 // [32]
+    unsigned int* wq = wword + 32;                                                     // [N_QUEUES][QUEUE_CAP]
     PolyBuf<32> poly{wpoly + lane};
 
     const Item item = A.items[blockIdx.x];
@@ -535,44 +540,18 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 wrect[lane] = rect;
                 wword[lane] = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
-            // ---- stage B: one pass per face (jobs of one pass never share a (tet, cell), so the
-            // shared atomics of a pass collide only between different tets); exclusive prefix of
-            // the face's job counts over the 32 slots
-            __syncwarp();
-#pragma unroll 1
-            for (int f = 0; f < 4; ++f) {
-            const int njobs = (cnts >> (8 * f)) & 255;
-            int pre = njobs;
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(0xffffffffu, pre, o);
-                if (lane >= o) pre += y;
-            }
-            const int total = __shfl_sync(0xffffffffu, pre, 31);
-            pre -= njobs;
-            for (int jb = 0; jb < total; jb += 32) {
-                const int job = jb + lane;
-                int slot = 0;  // largest slot with pre[slot] <= job
-#pragma unroll
-                for (int step = 16; step; step >>= 1) {
-                    int probe = __shfl_sync(0xffffffffu, pre, slot + step);
-                    if (probe <= job) slot += step;
-                }
-                const int spre = __shfl_sync(0xffffffffu, pre, slot);
-                // ---- stage C1: lane = face job.  Wall clip; the polygon stays in the lane's buffer.
+            // ---- stage C (a lambda: runs once per 32 queued jobs).  C1: lane = face job, wall clip
+            // (outcodes given), the polygon stays in the lane's buffer, trivial cells.  C2: the
+            // cutting planes (polygon, a) of the 32 jobs, numbered by a warp prefix sum, lane = plane;
+            // the kept part above the plane is integrated in closed form; +R to cell a, -R to a-1.
+            auto run_jobs = [&](const bool act, const unsigned int desc) {
                 unsigned int f_order = 0, f_info = 0;
                 int f_afirst = 0, k = 0;
                 double f_w = 0.0;
-                if (job < total) {
-                    // decode (slot, column)
+                if (act) {
+                    const int slot = desc & 31, f = (desc >> 5) & 3, cv = (desc >> 7) & 7, cw = (desc >> 10) & 7;
+                    const unsigned int oc = (desc >> 13) & 0xfffu;
                     const unsigned int word = wword[slot];
-                    const int local = job - spre;
-                    const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
-                    const int nw = ((r16 >> 9) & 7) + 1;
-                    // local / nw for local < 64, nw <= 8 without an integer division:
-                    // (local * ceil(256 / nw)) >> 8 is exact there; the table holds ceil(256/nw) - 1
-                    const int inv = (int)((0x1f242a333f557fffull >> (8 * (nw - 1))) & 255ull) + 1;
-                    const int lq = (local * inv) >> 8;
-                    const int cv = (r16 & 7) + lq, cw = ((r16 >> 6) & 7) + (local - lq * nw);
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
                     // the face triangle, column-local, into slots 0..2 of the lane's polygon buffer
@@ -587,8 +566,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
                     }
                     f_w = ts[12 * 32];
-                    if (COUNT) cnt.jobs++;
-                    const FaceClip fc = face_clip<32>(poly);
+                    const unsigned int all_in = oc & (oc >> 4) & (oc >> 8) & 15u;
+                    const FaceClip fc = face_clip_oc<32, false>(poly, oc, all_in, 15u);
                     if (fc.n >= 3 && fc.ice > c_lo) {
                         if (COUNT) cnt.face_clips++;
                         const FaceRun fr = face_run(fc, c_lo, c_hi);
@@ -616,9 +595,6 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                                  (unsigned)fc.n << 17;
                     }
                 }
-                // ---- stage C2: the cutting planes (polygon, a) of the 32 jobs, numbered by a warp
-                // prefix sum; lane = plane.  The kept part above the plane is integrated in closed
-                // form; +R to cell a, -R to cell a-1.
                 __syncwarp();
                 int pre2 = k;
                 for (int o = 1; o < 32; o <<= 1) {
@@ -655,7 +631,93 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     }
                 }
                 __syncwarp();
-            }
+            };
+            // ---- stage B: the face jobs (slot, face, column) of the 32 slots, face by face, numbered
+            // by a warp prefix sum of the rectangle sizes; lane = job computes the outcodes of its
+            // triangle against its column and queues the job by CLIP CLASS (walls with a vertex
+            // beyond them: <= 2, 3, 4), so that the 32 jobs stage C takes from one queue clip about
+            // the same number of walls.  A queue runs as soon as it holds 32 jobs; the rest at the end.
+            // One loop with a single call site of stage C (its code is large): drain a queue that
+            // holds 32 jobs, else generate the next 32 jobs, at the end drain what is left.
+            __syncwarp();
+            int qn0 = 0, qn1 = 0, qn2 = 0;  // N_QUEUES = 3 queue lengths (warp-uniform)
+            int f = -1, jb = 0, total = 0, pre = 0;
+            bool flushing = false;
+#pragma unroll 1
+            for (;;) {
+                const int thr = flushing ? 1 : 32;
+                const int c = qn0 >= thr ? 0 : (qn1 >= thr ? 1 : (qn2 >= thr ? 2 : -1));
+                if (c >= 0) {
+                    const int have_n = c == 0 ? qn0 : (c == 1 ? qn1 : qn2);
+                    const int take = min(have_n, 32), left = have_n - take;
+                    if (c == 0) qn0 = left; else if (c == 1) qn1 = left; else qn2 = left;
+                    __syncwarp();
+                    run_jobs(lane < take, lane < take ? wq[c * QUEUE_CAP + left + lane] : 0u);
+                    continue;
+                }
+                if (flushing) break;
+                if (jb >= total) {  // next face: exclusive prefix of its job counts over the 32 slots
+                    if (++f == 4) { flushing = true; continue; }
+                    const int njobs = (cnts >> (8 * f)) & 255;
+                    pre = njobs;
+                    for (int o = 1; o < 32; o <<= 1) {
+                        int y = __shfl_up_sync(0xffffffffu, pre, o);
+                        if (lane >= o) pre += y;
+                    }
+                    total = __shfl_sync(0xffffffffu, pre, 31);
+                    pre -= njobs;
+                    jb = 0;
+                    continue;
+                }
+                const int job = jb + lane;
+                jb += 32;
+                int slot = 0;  // largest slot with pre[slot] <= job
+#pragma unroll
+                for (int step = 16; step; step >>= 1) {
+                    int probe = __shfl_sync(0xffffffffu, pre, slot + step);
+                    if (probe <= job) slot += step;
+                }
+                const int spre = __shfl_sync(0xffffffffu, pre, slot);
+                unsigned int desc = 0;
+                int cls = -1;
+                if (job < total) {
+                    // decode (slot, column)
+                    const unsigned int word = wword[slot];
+                    const int local = job - spre;
+                    const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
+                    const int nw = ((r16 >> 9) & 7) + 1;
+                    // local / nw for local < 64, nw <= 8 without an integer division:
+                    // (local * ceil(256 / nw)) >> 8 is exact there; the table holds ceil(256/nw) - 1
+                    const int inv = (int)((0x1f242a333f557fffull >> (8 * (nw - 1))) & 255ull) + 1;
+                    const int lq = (local * inv) >> 8;
+                    const int cv = (r16 & 7) + lq, cw = ((r16 >> 6) & 7) + (local - lq * nw);
+                    const int ax = word & 3;
+                    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
+                    const double* ts = wtet + slot;
+                    const unsigned int fv = FACE_TABLE >> (6 * f);
+                    const double ov = (double)cv, ow = (double)cw;
+                    unsigned int oc = 0, all_in = 15u;
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) {
+                        const int vi = (fv >> (2 * i)) & 3;
+                        const double v = ts[(3 * vi + av) * 32] - ov, w = ts[(3 * vi + aw) * 32] - ow;
+                        const unsigned int o = (unsigned)(v >= 0.0) | (unsigned)(v <= 1.0) << 1 |
+                                               (unsigned)(w >= 0.0) << 2 | (unsigned)(w <= 1.0) << 3;
+                        oc |= o << (4 * i);
+                        all_in &= o;
+                    }
+                    if (COUNT) cnt.jobs++;
+                    const int pc = __popc(all_in ^ 15u);
+                    cls = pc <= 2 ? 0 : (pc == 3 ? 1 : 2);
+                    desc = (unsigned)slot | (unsigned)f << 5 | (unsigned)cv << 7 | (unsigned)cw << 10 | oc << 13;
+                }
+                const unsigned int lt = (1u << lane) - 1u;
+                const unsigned int m0 = __ballot_sync(0xffffffffu, cls == 0), m1 = __ballot_sync(0xffffffffu, cls == 1);
+                const unsigned int m2 = __ballot_sync(0xffffffffu, cls == 2);
+                if (cls == 0) wq[0 * QUEUE_CAP + qn0 + __popc(m0 & lt)] = desc;
+                if (cls == 1) wq[1 * QUEUE_CAP + qn1 + __popc(m1 & lt)] = desc;
+                if (cls == 2) wq[2 * QUEUE_CAP + qn2 + __popc(m2 & lt)] = desc;
+                qn0 += __popc(m0); qn1 += __popc(m1); qn2 += __popc(m2);
             }
         }
     }
