@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                     atomicAdd(&sh_stat[ST_SUM_CELLS], (unsigned long long)nc);
                     atomicMax(&sh_stat[ST_MAX_CELLS], (unsigned long long)nc);
                     atomicAdd(&sh_hist[0][bit_width_u64((unsigned long long)(nc - 1))], 1u);
-                    double det = tet_det(t.g);
+                    double det = tet_det_sign(t.g);
                     if (det < 0.0) atomicAdd(&sh_stat[ST_INVERTED], 1ull);
                     if (det == 0.0) atomicAdd(&sh_stat[ST_DEGENERATE], 1ull);
                 }
@@ -886,7 +886,7 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
         finish_tet(P, scale, t);
         nc = (unsigned long long)((long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) * (t.hi[2] - t.lo[2] + 1));
         atomicAdd(&sh_hist[bit_width_u64(nc - 1)], 1u);
-        double det = tet_det(t.g);
+        double det = tet_det_sign(t.g);
         inv = det < 0.0; deg = det == 0.0;
     }
     // warp partials (64-bit sum and max by halves), then one shared atomic per warp
