@@ -143,6 +143,9 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
     const int N = p.N;
     const int64_t ncell = (int64_t)N * N * N;
     int64_t cell = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    // statistics are summed per thread over its 6 tets, then per warp, then one shared atomic each
+    unsigned long long t_sum = 0, t_max = 0;
+    unsigned int t_inv = 0, t_deg = 0, t_pairs = 0, t_suspect = 0;
     if (cell < ncell) {
         int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((int64_t)N * N));
         double C[8][3];
@@ -157,7 +160,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                 if (!SCATTER && (b == 1 || b == 2 || b == 4))
                     suspect |= fabs(C[b][x] - C[0][x]) > 0.25 * p.L;
             }
-        if (!SCATTER && suspect) atomicAdd(&sh_stat[ST_UNWRAP], 1ull);
+        t_suspect = suspect;
         const int nlev = s.patch_mode ? s.n_levels : 1;
         for (int level = 0; level < nlev; ++level) {
             const double scale = level_scale(s, level);
@@ -177,12 +180,12 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                 if (!SCATTER && level == 0) {
                     long long nc = (long long)(t.hi[0] - t.lo[0] + 1) * (t.hi[1] - t.lo[1] + 1) *
                                    (t.hi[2] - t.lo[2] + 1);
-                    atomicAdd(&sh_stat[ST_SUM_CELLS], (unsigned long long)nc);
-                    atomicMax(&sh_stat[ST_MAX_CELLS], (unsigned long long)nc);
+                    t_sum += (unsigned long long)nc;
+                    t_max = (unsigned long long)nc > t_max ? (unsigned long long)nc : t_max;
                     atomicAdd(&sh_hist[0][bit_width_u64((unsigned long long)(nc - 1))], 1u);
                     double det = tet_det_sign(t.g);
-                    if (det < 0.0) atomicAdd(&sh_stat[ST_INVERTED], 1ull);
-                    if (det == 0.0) atomicAdd(&sh_stat[ST_DEGENERATE], 1ull);
+                    t_inv += det < 0.0;
+                    t_deg += det == 0.0;
                 }
                 for_each_block(t.lo, t.hi, Gl, TILE, nb, [&](int tx, int ty, int tz, long long inside) {
                     long long id = tile_id_of(s, level, tx, ty, tz);
@@ -192,7 +195,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                     if (!SCATTER) {
                         const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
                         if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&tile_counts[bin], (unsigned int)__popc(peers));
-                        atomicAdd(&sh_stat[ST_PAIRS], 1ull);
+                        ++t_pairs;
                         atomicAdd(&sh_hist[1][bit_width_u64((unsigned long long)(inside - 1))], 1u);
                     } else {
                         unsigned int slot = atomicAdd(&cursors[bin], 1u);
@@ -203,6 +206,23 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
         }
     }
     if (!SCATTER) {
+        for (int o = 16; o; o >>= 1) {
+            t_sum += __shfl_down_sync(0xffffffffu, t_sum, o);
+            const unsigned long long y = __shfl_down_sync(0xffffffffu, t_max, o);
+            t_max = y > t_max ? y : t_max;
+        }
+        t_inv = __reduce_add_sync(0xffffffffu, t_inv);
+        t_deg = __reduce_add_sync(0xffffffffu, t_deg);
+        t_pairs = __reduce_add_sync(0xffffffffu, t_pairs);
+        t_suspect = __reduce_add_sync(0xffffffffu, t_suspect);
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(&sh_stat[ST_SUM_CELLS], t_sum);
+            atomicMax(&sh_stat[ST_MAX_CELLS], t_max);
+            if (t_inv) atomicAdd(&sh_stat[ST_INVERTED], (unsigned long long)t_inv);
+            if (t_deg) atomicAdd(&sh_stat[ST_DEGENERATE], (unsigned long long)t_deg);
+            if (t_pairs) atomicAdd(&sh_stat[ST_PAIRS], (unsigned long long)t_pairs);
+            if (t_suspect) atomicAdd(&sh_stat[ST_UNWRAP], (unsigned long long)t_suspect);
+        }
         __syncthreads();
         for (int i = threadIdx.x; i < 128; i += blockDim.x) {
             unsigned int v = (&sh_hist[0][0])[i];
