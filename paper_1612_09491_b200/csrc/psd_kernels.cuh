@@ -198,7 +198,13 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                         ++t_pairs;
                         atomicAdd(&sh_hist[1][bit_width_u64((unsigned long long)(inside - 1))], 1u);
                     } else {
-                        unsigned int slot = atomicAdd(&cursors[bin], 1u);
+                        // one cursor atomic per distinct bin among the lanes that are here together
+                        const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
+                        const int leader = __ffs(peers) - 1;
+                        unsigned int base = 0;
+                        if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&cursors[bin], (unsigned int)__popc(peers));
+                        base = __shfl_sync(peers, base, leader);
+                        const unsigned int slot = base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u));
                         pair_ids[tile_offsets[bin] + slot] = tet_id;
                     }
                 });
