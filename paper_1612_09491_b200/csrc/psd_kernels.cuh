@@ -463,7 +463,9 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
         // periodic image of the tile it meets (almost always one), so that nothing of stage A stays
         // in registers across stages B and C.
         const bool have = base + lane < item.count;
-        const unsigned int id = have ? A.pair_ids[item.begin + base + lane] : 0u;
+        // the list is taken from its end: the large class first, the small pairs last, so that the
+        // warps of the CTA reach the end-of-item barrier closer together
+        const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - (base + lane))] : 0u;
         int max_images = 1;
         for (int img = 0; img < max_images; ++img) {
             // ---- stage A: slot = lane.  Tile-local vertices, weight, face rectangles.
