@@ -606,14 +606,24 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         const int colofs = cv * sv + cw * sw;
                         // trivial part: cells entirely below Q get its projected area, the cell
                         // holding umin gets M1 - c A
+                        {
+                            const int full_hi = min(fr.t_hi, fc.ifl - 1);  // cells entirely below Q
+                            const double wA = f_w * fc.A;
+                            if (wA != 0.0) {
 #pragma unroll
-                        for (int cc = 0; cc < TILE; ++cc) {
-                            const int c = c_lo + cc;
-                            if (c > fr.t_hi) break;
-                            const double D = c + 1 <= fc.ifl ? fc.A : fma(-(double)c, fc.A, fc.M1);
-                            if (D != 0.0) {
-                                atomicAdd(acc + colofs + c * su, f_w * D);
-                                if (COUNT) cnt.cells++;
+                                for (int cc = 0; cc < TILE; ++cc) {
+                                    const int c = c_lo + cc;
+                                    if (c > full_hi) break;
+                                    atomicAdd(acc + colofs + c * su, wA);
+                                    if (COUNT) cnt.cells++;
+                                }
+                            }
+                            if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {  // the cell holding umin
+                                const double D = fma(-(double)fc.ifl, fc.A, fc.M1);
+                                if (D != 0.0) {
+                                    atomicAdd(acc + colofs + fc.ifl * su, f_w * D);
+                                    if (COUNT) cnt.cells++;
+                                }
                             }
                         }
                         k = max(fr.a_last - fr.a_first + 1, 0);
