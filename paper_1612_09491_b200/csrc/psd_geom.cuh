@@ -469,9 +469,12 @@ __device__ __forceinline__ void face_job(PolyBuf<S> q, int c_lo, int c_hi, Emit 
     const FaceRun fr = face_run(fc, c_lo, c_hi);
     if (fc.n < 3 || fc.ice <= c_lo) return;
     if (COUNT) cnt->face_clips++;
-    for (int c = c_lo; c <= fr.t_hi; ++c) {
-        const double D = c + 1 <= fc.ifl ? fc.A : fma(-(double)c, fc.A, fc.M1);
-        if (D != 0.0) { emit(c, D); if (COUNT) cnt->cells++; }
+    const int full_hi = min(fr.t_hi, fc.ifl - 1);  // cells entirely below Q: its projected area
+    if (fc.A != 0.0)
+        for (int c = c_lo; c <= full_hi; ++c) { emit(c, fc.A); if (COUNT) cnt->cells++; }
+    if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {      // the cell holding umin
+        const double D = fma(-(double)fc.ifl, fc.A, fc.M1);
+        if (D != 0.0) { emit(fc.ifl, D); if (COUNT) cnt->cells++; }
     }
     for (int a = fr.a_first; a <= fr.a_last; ++a) {
         const double R = plane_integral6<S>(q, fc.order, fc.n, (double)a) * (1.0 / 6.0);
