@@ -168,8 +168,10 @@ PSD_API int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int
                         int base_G, double* mass_dev, int accumulate);
 
 /* End-to-end convenience used for the host-buffer measurement: copies positions host->device,
- * registers them, deposits, copies the G^3 grid device->host.  Synchronous.  Host buffers
- * should be pinned for full copy bandwidth. */
+ * registers them, deposits, copies the G^3 grid device->host.  On the binned path the grid goes
+ * back in up to 8 slabs of x-tiles, each copied (on a second stream) as soon as the work items
+ * of its tiles are done, while the later slabs are still being deposited.  Synchronous.  Host
+ * buffers should be pinned for full copy bandwidth and for the overlap. */
 PSD_API int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
                              double L, double total_mass, int G, double* grid_host);
 

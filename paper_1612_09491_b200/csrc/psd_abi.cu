@@ -53,6 +53,13 @@ struct psd_ctx {
     std::string err;
     int64_t launches = 0;
     cudaEvent_t ev[6] = {};
+    // psd_deposit_uniform_host: the grid goes back to the host slab by slab while later slabs are
+    // still being deposited (copy stream + one event per slab)
+    static constexpr int MAX_SLABS = 8;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t slab_ev[MAX_SLABS] = {}, copy_done = nullptr;
+    double* stream_out_host = nullptr;  // set only inside psd_deposit_uniform_host
+    bool streamed = false;              // run_binned copied the grid itself
 };
 
 namespace {
@@ -71,7 +78,7 @@ int cuda_fail(psd_ctx* c, cudaError_t e, const char* what) {
         if (_e != cudaSuccess) return cuda_fail(ctx, _e, #call);    \
     } while (0)
 
-constexpr int PINNED_WORDS = ST_COUNT + 128 + 2;
+constexpr int PINNED_WORDS = ST_COUNT + 128 + 2 + psd_ctx::MAX_SLABS + 1;
 
 int reset_stats(psd_ctx* ctx) {
     CK(ctx->stats.ensure(sizeof(unsigned long long) * ST_COUNT));
@@ -123,6 +130,17 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     // the only host round trip of a deposit: list sizes, to size the scratch and the grid
     CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 128, ctx->totals.p, sizeof(unsigned long long) * 2,
                        cudaMemcpyDeviceToHost, st));
+    // host-output mode (uniform grid): the first work item of each slab of x-tiles
+    int n_slabs = 0;
+    if (ctx->stream_out_host && !space.patch_mode) {
+        // few slabs for small grids: every launch ends in a partly filled wave
+        n_slabs = space.nt / 8 < 1 ? 1 : (space.nt / 8 < psd_ctx::MAX_SLABS ? space.nt / 8 : psd_ctx::MAX_SLABS);
+        for (int sl = 1; sl < n_slabs; ++sl) {
+            const long long bin = (long long)(sl * space.nt / n_slabs) * space.nt * space.nt * N_CLASSES;
+            CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + sl, ctx->item_offsets.as<unsigned long long>() + bin,
+                               sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        }
+    }
     CK(cudaStreamSynchronize(st));
     const unsigned long long n_pairs = ctx->pinned[ST_COUNT + 128], n_items = ctx->pinned[ST_COUNT + 129];
     ctx->last.n_pairs = (int64_t)n_pairs;
@@ -150,6 +168,37 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         A.weight_mode = ctx->weight_mode;
         A.chord_axis = ctx->chord_axis;
         A.stats = ctx->stats.as<unsigned long long>();
+        if (n_slabs > 1) {
+            // one launch per slab of x-tiles (items are in tile order); the finished slab of the grid
+            // goes to the host on the copy stream while the next slabs are deposited
+            unsigned long long* ib = ctx->pinned + ST_COUNT + 130;
+            ib[0] = 0; ib[n_slabs] = n_items;
+            const Item* items0 = A.items;
+            const size_t plane = sizeof(double) * (size_t)space.G * space.G;
+            for (int sl = 0; sl < n_slabs; ++sl) {
+                const unsigned int cnt = (unsigned int)(ib[sl + 1] - ib[sl]);
+                if (cnt) {
+                    A.items = items0 + ib[sl];
+                    if (ctx->counters) k_deposit_tiles<true><<<cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                    else k_deposit_tiles<false><<<cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                    ctx->launches += 1;
+                }
+                CK(cudaEventRecord(ctx->slab_ev[sl], st));
+                CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_ev[sl], 0));
+                const size_t x0 = (size_t)(sl * space.nt / n_slabs) * TILE, x1 = (size_t)((sl + 1) * space.nt / n_slabs) * TILE;
+                CK(cudaMemcpyAsync(reinterpret_cast<char*>(ctx->stream_out_host) + x0 * plane,
+                                   reinterpret_cast<const char*>(space.out) + x0 * plane, (x1 - x0) * plane,
+                                   cudaMemcpyDeviceToHost, ctx->copy_stream));
+            }
+            CK(cudaEventRecord(ctx->copy_done, ctx->copy_stream));
+            CK(cudaEventRecord(ctx->ev[4], st));  // the deposit's own time ends here
+            CK(cudaStreamWaitEvent(st, ctx->copy_done, 0));
+            ctx->streamed = true;
+            CK(cudaGetLastError());
+            ctx->stats_pending = true;
+            ctx->binned_last = true;
+            return PSD_OK;
+        }
         if (ctx->counters)
             k_deposit_tiles<true><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
         else
@@ -217,6 +266,10 @@ int psd_create(psd_ctx** out, int device, void* cuda_stream) {
     e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->pinned, sizeof(unsigned long long) * PINNED_WORDS);
     for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreate(&ctx->ev[i]);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < psd_ctx::MAX_SLABS && e == cudaSuccess; ++i)
+        e = cudaEventCreateWithFlags(&ctx->slab_ev[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->copy_done, cudaEventDisableTiming);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_deposit_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
     if (e == cudaSuccess)
@@ -240,6 +293,10 @@ void psd_destroy(psd_ctx* ctx) {
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 6; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    for (int i = 0; i < psd_ctx::MAX_SLABS; ++i)
+        if (ctx->slab_ev[i]) cudaEventDestroy(ctx->slab_ev[i]);
+    if (ctx->copy_done) cudaEventDestroy(ctx->copy_done);
     delete ctx;
 }
 
@@ -470,9 +527,13 @@ int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int 
     CK(cudaMemcpyAsync(ctx->host_pos.p, pos_host, pbytes, cudaMemcpyHostToDevice, ctx->stream));
     int rc = psd_build_tets(ctx, ctx->host_pos.p, dtype, stride_elems, N, L, total_mass);
     if (rc) return rc;
+    ctx->stream_out_host = grid_host;
+    ctx->streamed = false;
     rc = psd_deposit_uniform(ctx, G, ctx->host_grid.as<double>(), 0);
+    ctx->stream_out_host = nullptr;
     if (rc) return rc;
-    CK(cudaMemcpyAsync(grid_host, ctx->host_grid.p, gbytes, cudaMemcpyDeviceToHost, ctx->stream));
+    if (!ctx->streamed)  // direct path, or nothing to deposit: one copy at the end
+        CK(cudaMemcpyAsync(grid_host, ctx->host_grid.p, gbytes, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return PSD_OK;
 }
