@@ -310,6 +310,16 @@ def test_host_buffer_entry_point(psd, ctx, oracle):
     ctx.psd_deposit_uniform_host(hp, 24, hg)
     assert_parity(hg.numpy(), ora)
     assert ctx.psd_launch_count() > 0
+    # G = 192 (24 tiles per side): the grid comes back in 3 slabs of x-tiles on the copy stream while
+    # later slabs are deposited; every cell against the oracle, twice (the context's buffers are reused)
+    pos = crossing_field(24, 1.5, dtype="float32", stride=4)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 192)
+    hp = torch.from_numpy(pos).pin_memory()
+    hg = torch.full((192, 192, 192), -1.0, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        ctx.psd_deposit_uniform_host(hp, 192, hg)
+        assert_parity(hg.numpy(), ora)
+        hg.fill_(-1.0)
 
 
 def test_runs_on_a_non_default_stream(psd, oracle):
