@@ -435,17 +435,20 @@ int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double fa
     CK(ctx->refine_counts.ensure(sizeof(unsigned long long) * (size_t)(off[nl] + 1)));
     CK(cudaMemsetAsync(ctx->refine_counts.p, 0, sizeof(unsigned long long) * (size_t)(off[nl] + 1), ctx->stream));
     const long long ntet = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
-    for (int l = 0; l < nl; ++l) {
-        unsigned long long* dst = ctx->refine_counts.as<unsigned long long>() + off[l];
-        if (ctx->refine_subblock > 0) {  // estimate from sub-block bounding boxes
+    if (ctx->refine_subblock > 0) {  // estimate from sub-block bounding boxes
+        for (int l = 0; l < nl; ++l) {
             const int B = ctx->refine_subblock;
             const long long nb = (ctx->part.N + B - 1) / B;
             k_subblock_counts<<<(unsigned int)((nb * nb * nb + 3) / 4), 128, 0, ctx->stream>>>(
-                ctx->part, base_G, P, l, B, dst,
+                ctx->part, base_G, P, l, B, ctx->refine_counts.as<unsigned long long>() + off[l],
                 reinterpret_cast<unsigned int*>(ctx->refine_counts.as<unsigned long long>() + off[nl]));
-        } else {  // every tet counted
-            k_patch_counts<<<(unsigned int)((ntet + 255) / 256), 256, 0, ctx->stream>>>(ctx->part, base_G, P, l, dst);
+            ctx->launches += 1;
         }
+    } else {  // every tet counted, all levels in one pass over the tets
+        LevelOffsets lo{};
+        for (int l = 0; l < nl; ++l) lo.off[l] = off[l];
+        k_patch_counts<<<(unsigned int)((ntet + 255) / 256), 256, 0, ctx->stream>>>(
+            ctx->part, base_G, P, nl, ctx->refine_counts.as<unsigned long long>(), lo);
         ctx->launches += 1;
     }
     CK(cudaGetLastError());

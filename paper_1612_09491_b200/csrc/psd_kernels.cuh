@@ -953,24 +953,28 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
 // ---------------------------------------------------------------- a7 refinement census
 // counts[level] (dense, (base_G/P * 2^level)^3): tets whose cell range on the level grid meets
 // each candidate patch position, each position once per tet.
-__global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, int P, int level,
-                                                      unsigned long long* counts) {
+struct LevelOffsets { long long off[8]; };  // start of each level's dense count array
+__global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, int P, int n_levels,
+                                                      unsigned long long* counts, LevelOffsets lo) {
     int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (id >= ntet) return;
-    const int Gl = base_G << level;
-    const int np = Gl / P;
     double V[4][3];
-    load_tet_vertices(p, id / 6, (int)(id % 6), V);
-    Tet t;
-    finish_tet(V, __ddiv_rn((double)Gl, p.L), t);
-    // neighbouring tets mostly meet the same positions: one atomic per distinct position among the
-    // lanes that are here together
-    for_each_block(t.lo, t.hi, Gl, P, np, [&](int bx, int by, int bz, long long) {
-        const unsigned int key = (unsigned int)(((long long)bx * np + by) * np + bz);
-        const unsigned int peers = __match_any_sync(__activemask(), key);
-        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&counts[key], (unsigned long long)__popc(peers));
-    });
+    load_tet_vertices(p, id / 6, (int)(id % 6), V);  // once for all levels
+    for (int level = 0; level < n_levels; ++level) {
+        const int Gl = base_G << level;
+        const int np = Gl / P;
+        unsigned long long* cl = counts + lo.off[level];
+        Tet t;
+        finish_tet(V, __ddiv_rn((double)Gl, p.L), t);
+        // neighbouring tets mostly meet the same positions: one atomic per distinct position among
+        // the lanes that are here together
+        for_each_block(t.lo, t.hi, Gl, P, np, [&](int bx, int by, int bz, long long) {
+            const unsigned int key = (unsigned int)(((long long)bx * np + by) * np + bz);
+            const unsigned int peers = __match_any_sync(__activemask(), key);
+            if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&cl[key], (unsigned long long)__popc(peers));
+        });
+    }
 }
 
 // a7: the memory-lean census.  One warp per sub-block of B^3 Lagrangian cells:
