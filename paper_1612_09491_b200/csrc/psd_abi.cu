@@ -381,6 +381,10 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
     s.base_G = base_G;
     s.P = P;
     s.tp = P / TILE;
+    s.np0 = base_G / P;
+    s.tp_shift = -1;
+    for (int k = 0; k < 16; ++k)
+        if ((1 << k) == s.tp) s.tp_shift = k;
     s.n_levels = max_level + 1;
     s.L = ctx->part.L;
     s.out = mass_dev;

@@ -19,6 +19,7 @@ struct Space {
     int nt;           // tiles per side (G/8), binned path only
     // patches
     int base_G, P, tp;        // tp = P/8 tiles per patch side
+    int tp_shift, np0;        // log2(tp) or -1; np0 = base_G / P patch positions per side on level 0
     int n_levels;
     const PatchDev* patches;  // device
     const int* lookup;        // dense patch-position -> patch index (or -1), levels concatenated
@@ -115,12 +116,19 @@ __device__ __forceinline__ void for_each_block(const int lo[3], const int hi[3],
 // tile id of wrapped tile coords on `level`; -1 if no patch there (patch mode)
 __device__ __forceinline__ long long tile_id_of(const Space& s, int level, int tx, int ty, int tz) {
     if (!s.patch_mode) return ((long long)tx * s.nt + ty) * s.nt + tz;
-    int np = (s.base_G << level) / s.P;
-    int px = tx / s.tp, py = ty / s.tp, pz = tz / s.tp;
-    int pi = s.lookup[s.lookup_off[level] + ((long long)px * np + py) * np + pz];
+    const int np = s.np0 << level;  // patch positions per side: (base_G / P) * 2^level
+    int px, py, pz, sx, sy, sz;
+    if (s.tp_shift >= 0) {  // tiles per patch side a power of two: no integer division
+        const int m = s.tp - 1;
+        px = tx >> s.tp_shift; py = ty >> s.tp_shift; pz = tz >> s.tp_shift;
+        sx = tx & m; sy = ty & m; sz = tz & m;
+    } else {
+        px = tx / s.tp; py = ty / s.tp; pz = tz / s.tp;
+        sx = tx - px * s.tp; sy = ty - py * s.tp; sz = tz - pz * s.tp;
+    }
+    const int pi = s.lookup[s.lookup_off[level] + ((long long)px * np + py) * np + pz];
     if (pi < 0) return -1;
-    int sub = ((tx % s.tp) * s.tp + (ty % s.tp)) * s.tp + (tz % s.tp);
-    return (long long)pi * (s.tp * s.tp * s.tp) + sub;
+    return (long long)pi * (s.tp * s.tp * s.tp) + (sx * s.tp + sy) * s.tp + sz;
 }
 
 // ---------------------------------------------------------------- a2 census / a3 scatter
