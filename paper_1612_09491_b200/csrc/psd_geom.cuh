@@ -368,7 +368,7 @@ struct FaceClip {
 
 // q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
 // corner (the column is the unit square [0,1]^2).
-// outcodes of the triangle in slots 0..2 (nibble i = vertex i, see PolyRef::oc), their AND and OR
+// tri_outcodes: outcodes of that triangle (nibble i = vertex i, see PolyRef::oc), their AND and OR.
 template <int S>
 __device__ __forceinline__ unsigned tri_outcodes(PolyBuf<S> q, unsigned& all_in, unsigned& any_in) {
     unsigned oc = 0;
