@@ -320,6 +320,10 @@ def test_host_buffer_entry_point(psd, ctx, oracle):
         ctx.psd_deposit_uniform_host(hp, 192, hg)
         assert_parity(hg.numpy(), ora)
         hg.fill_(-1.0)
+    # pageable host memory (plain numpy arrays): the copies serialise but the result is the same
+    ng = np.full((192, 192, 192), -1.0)
+    ctx.psd_deposit_uniform_host(pos, 192, ng)
+    assert_parity(ng, ora)
 
 
 def test_runs_on_a_non_default_stream(psd, oracle):
