@@ -252,3 +252,147 @@ def test_fp32_geometry_does_not_hold_the_parity_tolerance(oracle):
     assert (np.abs(dbl - gold) / tol).max() < 1e-3
     assert (np.abs(sgl - gold) / tol).max() > 5.0
     assert abs(sgl.sum() - 1.0) > 1e-10 > abs(dbl.sum() - 1.0)
+
+
+# ------------------------------------------------------------------ O5 / O6 / Q14: pins of the counters
+def _bit_width(v: int) -> int:
+    return int(v).bit_length()
+
+
+def _clustered(x, y, z):
+    """N = 2 'lattice' whose per-axis coordinates are the given pairs: every Lagrangian cell has
+    the same bounding box [min, max] per axis (the wrap cell unwraps back to it), and every Kuhn
+    tet holds corners 0 and 7, hence spans that whole box."""
+    pos = np.empty((2, 2, 2, 3))
+    pos[..., 0] = np.asarray(x)[:, None, None]
+    pos[..., 1] = np.asarray(y)[None, :, None]
+    pos[..., 2] = np.asarray(z)[None, None, :]
+    return pos
+
+
+@pytest.mark.parametrize("x,y,z,ncell,bucket", [
+    ((0.30, 0.31), (0.30, 0.31), (0.30, 0.31), 1, 0),        # all in cell (1,1,1) of G = 4
+    ((0.249, 0.251), (0.30, 0.31), (0.30, 0.31), 2, 1),      # straddles x = 1/4
+    ((0.249, 0.251), (0.499, 0.501), (0.749, 0.751), 8, 3),  # straddles one face per axis
+    ((0.249, 0.501), (0.249, 0.501), (0.30, 0.31), 9, 4),    # 3 x 3 x 1 cells
+])
+def test_census_histogram_buckets_hand_made(oracle, x, y, z, ncell, bucket):
+    """O5: bucket b = bit_width(n_cells - 1): ranges of 1, 2, 8, 9 cells fall in buckets 0, 1, 3, 4
+    (worked out by hand from the coordinates, G = 4, tile = 2)."""
+    c = oracle.census(_clustered(x, y, z), 1.0, 4, tile=2)
+    want = np.zeros(64, dtype=np.uint64)
+    want[bucket] = 48
+    assert np.array_equal(c["hist_tet"], want)
+    assert c["sum_cells"] == 48 * ncell and c["max_cells"] == ncell
+
+
+def test_census_pair_histogram_hand_made(oracle):
+    """O5, per (tet, tile) pair: the 3 x 3 x 1 range above covers cells 0..2 in x and y, i.e. 2 cells
+    of tile 0 and 1 cell of tile 1 per axis, and one z cell (cell 1, tile 0): pairs of
+    4, 2, 2 and 1 cells -> buckets bit_width(n-1) = 2, 1, 1, 0, one of each per tet."""
+    c = oracle.census(_clustered((0.249, 0.501), (0.249, 0.501), (0.30, 0.31)), 1.0, 4, tile=2)
+    want = np.zeros(64, dtype=np.uint64)
+    want[0], want[1], want[2] = 48, 96, 48
+    assert np.array_equal(c["hist_pair"], want)
+    tc = c["tile_counts"].reshape(2, 2, 2)
+    assert np.array_equal(tc[:, :, 0], np.full((2, 2), 48)) and not tc[:, :, 1].any()
+    assert c["n_pairs"] == 4 * 48
+
+
+def test_census_histograms_recomputed_in_python(oracle):
+    """O5: hist_tet, hist_pair and the per-tile 'inside' counts recomputed with python sets from
+    the single-tet entry point on a crossing field whose tets wrap around the box."""
+    N, G, tile = 8, 16, 8
+    pos = crossing_field(N, 2.0)
+    c = oracle.census(pos, 1.0, G)
+    ht, hp = np.zeros(64, dtype=np.uint64), np.zeros(64, dtype=np.uint64)
+    for i in range(N):
+        for j in range(N):
+            for k in range(N):
+                for t in range(6):
+                    _, _, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+                    n = [int(hi[a] - lo[a] + 1) for a in range(3)]
+                    ht[_bit_width(n[0] * n[1] * n[2] - 1)] += 1
+                    per_axis = []
+                    for a in range(3):
+                        inside = {}
+                        for cc in range(int(lo[a]), int(hi[a]) + 1):
+                            inside[(cc % G) // tile] = inside.get((cc % G) // tile, 0) + 1
+                        per_axis.append(inside)
+                    for na in per_axis[0].values():
+                        for nb in per_axis[1].values():
+                            for nc in per_axis[2].values():
+                                hp[_bit_width(na * nb * nc - 1)] += 1
+    assert np.array_equal(ht, c["hist_tet"])
+    assert np.array_equal(hp, c["hist_pair"])
+    assert np.count_nonzero(hp) >= 4      # the field does spread over several buckets
+
+
+def test_patch_stats_counters_recomputed_per_tet(oracle):
+    """O6 counters (they feed bench.py's work model for the patch config): candidate cells of a
+    patch = cells of each tet's range that wrap into the patch box; cells with non-zero overlap
+    counted with the single-tet entry point."""
+    N, base_G, P = 6, 8, 4
+    pos = crossing_field(N, 1.2)
+    patches = np.array([[0, 0, 0, 0], [0, 1, 0, 1], [1, 3, 0, 2], [1, 0, 3, 3]], dtype=np.int32)
+    _, st = oracle.deposit_patches_stats(pos, 1.0, 1.0, base_G, P, patches)
+    want = np.zeros((len(patches), 2), dtype=np.int64)
+    for q, (lv, ox, oy, oz) in enumerate(patches.tolist()):
+        G = base_G << lv
+        org = (ox * P, oy * P, oz * P)
+        for i in range(N):
+            for j in range(N):
+                for k in range(N):
+                    for t in range(6):
+                        verts, _, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+                        n = (hi - lo + 1).astype(np.int64)
+                        vol, _ = oracle.tet_deposit_box(verts * float(G), lo, n)
+                        sel = np.ones(tuple(n), dtype=bool)
+                        for a in range(3):
+                            cells = (np.arange(lo[a], hi[a] + 1) % G)
+                            ok = (cells >= org[a]) & (cells < org[a] + P)
+                            sel &= ok.reshape([-1 if b == a else 1 for b in range(3)])
+                        want[q, 0] += int(sel.sum())
+                        want[q, 1] += int(((vol != 0) & sel).sum())
+    assert np.array_equal(st, want)
+    assert (want[:, 1] > 0).all() and (want[:, 1] < want[:, 0]).all()
+
+
+def test_refine_rule_literal_top_down_hand_built():
+    """Q14, rule 0 on hand-built counts with a known answer: threshold = factor x mean of level 0;
+    a patch above it is split, its children are tested against the SAME absolute number."""
+    from oracle import psd_oracle as oracle
+    c0 = np.array([10, 10, 10, 10, 10, 10, 10, 50], dtype=np.uint64).reshape(2, 2, 2)  # mean 15
+    c1 = np.zeros((4, 4, 4), dtype=np.uint64)
+    c1[2:, 2:, 2:] = 5            # children of (1,1,1)
+    c1[3, 3, 3] = 40              # one of them above 2 x 15 = 30
+    c1[0, 0, 0] = 1000            # far above, but its parent (0,0,0) is not split: must not appear
+    c2 = np.zeros((8, 8, 8), dtype=np.uint64)
+    pl = oracle.refine_patches([c0, c1, c2], 2.0, rule=oracle.RULE_LITERAL_TOP_DOWN)
+    got = {tuple(r) for r in pl.tolist()}
+    want = {(0, a, b, c) for a in range(2) for b in range(2) for c in range(2)}
+    want |= {(1, 2 + a, 2 + b, 2 + c) for a in range(2) for b in range(2) for c in range(2)}
+    want |= {(2, 6 + a, 6 + b, 6 + c) for a in range(2) for b in range(2) for c in range(2)}
+    assert got == want and len(pl) == len(want)
+    # the order is level, then (ox, oy, oz) lexicographic
+    assert pl.tolist() == sorted(pl.tolist())
+    # a count exactly AT the threshold does not split (strict >)
+    c0b = np.array([10, 10, 10, 10, 10, 10, 10, 30], dtype=np.uint64).reshape(2, 2, 2)  # mean 12.5
+    pl = oracle.refine_patches([c0b, c1], 2.4, rule=oracle.RULE_LITERAL_TOP_DOWN)      # thr = 30
+    assert len(pl) == 8
+
+
+def test_refine_rule_bottom_up_hand_built():
+    """Q14, rule 1 on hand-built counts: hot = count > factor x mean of ITS level; a parent is
+    split if any child is hot or split; splitting creates all 8 children."""
+    from oracle import psd_oracle as oracle
+    c0 = np.ones((2, 2, 2), dtype=np.uint64)
+    c1 = np.ones((4, 4, 4), dtype=np.uint64)
+    c2 = np.ones((8, 8, 8), dtype=np.uint64)
+    c2[5, 0, 2] = 600             # mean = (511 + 600) / 512 = 2.17; 600 > 4 x mean: hot
+    pl = oracle.refine_patches([c0, c1, c2], 4.0)
+    got = {tuple(r) for r in pl.tolist()}
+    want = {(0, a, b, c) for a in range(2) for b in range(2) for c in range(2)}
+    want |= {(1, 2 + a, b, c) for a in range(2) for b in range(2) for c in range(2)}      # children of (0,1,0,0)
+    want |= {(2, 4 + a, b, 2 + c) for a in range(2) for b in range(2) for c in range(2)}  # children of (1,2,0,1)
+    assert got == want
