@@ -175,6 +175,19 @@ PSD_API int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int
 PSD_API int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
                              double L, double total_mass, int G, double* grid_host);
 
+/* The same for the patch path with HOST buffers: copies
+ * the positions host->device, registers them, builds the patch list (psd_refine_patches with
+ * base_G, P, max_level, factor, rule), deposits into every listed patch and copies the masses
+ * device->host.
+ *   patches_out_host  receives the patch list (capacity cap patches); *n_out its length
+ *   mass_host         receives *n_out * P^3 doubles, patch-major then (x*P+y)*P+z; the caller
+ *                     provides room for cap * P^3 doubles
+ * PSD_ERR_INVALID_ARG (and *n_out = the length needed) when cap is too small.  Synchronous. */
+PSD_API int psd_deposit_patches_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N,
+                             double L, double total_mass, int base_G, int P, int max_level, double factor,
+                             int rule, psd_patch* patches_out_host, int64_t cap, int64_t* n_out,
+                             double* mass_host);
+
 /* Synchronises, then fills *out with the counters of the last build / deposit. */
 PSD_API int psd_get_stats(psd_ctx* ctx, psd_stats* out);
 

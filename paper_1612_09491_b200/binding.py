@@ -20,6 +20,7 @@ RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN = 0, 1
 # every symbol include/psd.h declares (tests check the library exports exactly these)
 EXPORTS = ("psd_create", "psd_destroy", "psd_build_tets", "psd_deposit_uniform",
            "psd_refine_patches", "psd_deposit_patches", "psd_deposit_uniform_host",
+           "psd_deposit_patches_host",
            "psd_get_stats", "psd_get_tile_counts", "psd_get_tile_class_counts", "psd_set_option", "psd_sync", "psd_last_error", "psd_launch_count",
            "psd_version")
 
@@ -80,6 +81,8 @@ def lib() -> C.CDLL:
                                      C.POINTER(i64), C.POINTER(C.c_uint64)]
     L.psd_deposit_patches.argtypes = [vp, C.POINTER(PsdPatch), i64, i, i, vp, i]
     L.psd_deposit_uniform_host.argtypes = [vp, vp, i, i, i, d, d, i, vp]
+    L.psd_deposit_patches_host.argtypes = [vp, vp, i, i, i, d, d, i, i, i, d, i, C.POINTER(PsdPatch), i64,
+                                           C.POINTER(i64), vp]
     L.psd_get_stats.argtypes = [vp, C.POINTER(PsdStats)]
     L.psd_get_tile_counts.argtypes = [vp, C.POINTER(C.c_uint32), i64]
     L.psd_get_tile_class_counts.argtypes = [vp, C.POINTER(C.c_uint32), i64]
@@ -207,14 +210,56 @@ class Context:
                                              base_G, mass_dev.data_ptr(), int(accumulate)))
         return mass_dev
 
+    @staticmethod
+    def _host_ptr(a, what: str, dtype_name: str | None = None, numel: int | None = None) -> int:
+        """Address of a C-contiguous HOST array (torch CPU tensor or numpy array), validated: the
+        library writes / reads it with raw copies, so a wrong dtype or size would corrupt memory."""
+        is_torch = hasattr(a, "data_ptr")
+        if is_torch:
+            if a.is_cuda:
+                raise ValueError(f"{what} must be a host (CPU) tensor")
+            contiguous, n = a.is_contiguous(), a.numel()
+        elif isinstance(a, np.ndarray):
+            contiguous, n = a.flags.c_contiguous, a.size
+        else:
+            raise TypeError(f"{what} must be a torch CPU tensor or a numpy array")
+        if not contiguous:
+            raise ValueError(f"{what} must be C-contiguous")
+        if dtype_name is not None and not str(a.dtype).endswith(dtype_name):
+            raise ValueError(f"{what} must be {dtype_name}, not {a.dtype}")
+        if numel is not None and n != numel:
+            raise ValueError(f"{what} must hold {numel} elements, not {n}")
+        if not is_torch and not a.flags.writeable and dtype_name is not None:
+            raise ValueError(f"{what} must be writeable")
+        return a.data_ptr() if is_torch else a.ctypes.data
+
     def psd_deposit_uniform_host(self, pos_host, G: int, grid_host, L: float = 1.0,
                                  total_mass: float = 1.0):
         """pos_host / grid_host: host (ideally pinned) torch tensors or numpy arrays."""
         dt, stride, N = _pos_meta(pos_host)
-        pp = pos_host.data_ptr() if hasattr(pos_host, "data_ptr") else pos_host.ctypes.data
-        gp = grid_host.data_ptr() if hasattr(grid_host, "data_ptr") else grid_host.ctypes.data
+        pp = self._host_ptr(pos_host, "pos_host")
+        gp = self._host_ptr(grid_host, "grid_host", "float64", int(G) ** 3)
         self._ck(self._L.psd_deposit_uniform_host(self._h, pp, dt, stride, N, L, total_mass, G, gp))
         return grid_host
+
+    def psd_deposit_patches_host(self, pos_host, base_G: int, P: int, max_level: int, factor: float,
+                                 mass_host, rule: int = RULE_BOTTOM_UP_LEVEL_MEAN, L: float = 1.0,
+                                 total_mass: float = 1.0):
+        """Host-buffer patch deposit: returns the (n, 4) int32 patch list; the masses of patch q
+        are mass_host.reshape(-1, P, P, P)[q].  mass_host: float64 host buffer whose capacity
+        (elements // P^3) bounds the number of patches."""
+        dt, stride, N = _pos_meta(pos_host)
+        pp = self._host_ptr(pos_host, "pos_host")
+        mp = self._host_ptr(mass_host, "mass_host", "float64")
+        n_el = mass_host.numel() if hasattr(mass_host, "numel") else mass_host.size
+        cap = int(n_el) // (P ** 3)
+        if cap < 1:
+            raise ValueError("mass_host has no room for a single patch")
+        out = (PsdPatch * cap)()
+        n = C.c_int64(0)
+        self._ck(self._L.psd_deposit_patches_host(self._h, pp, dt, stride, N, L, total_mass, base_G, P,
+                                                  max_level, factor, rule, out, cap, C.byref(n), mp))
+        return np.frombuffer(out, dtype=np.int32).reshape(cap, 4)[: n.value].copy()
 
     def psd_get_stats(self) -> PsdStats:
         s = PsdStats()

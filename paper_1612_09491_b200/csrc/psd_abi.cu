@@ -545,6 +545,31 @@ int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int 
     return PSD_OK;
 }
 
+int psd_deposit_patches_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N, double L,
+                             double total_mass, int base_G, int P, int max_level, double factor, int rule,
+                             psd_patch* patches_out_host, int64_t cap, int64_t* n_out, double* mass_host) {
+    if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
+    if (!pos_host || !patches_out_host || !n_out || !mass_host || cap < 1)
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_deposit_patches_host: NULL buffer or no capacity");
+    if ((dtype != PSD_F32 && dtype != PSD_F64) || (stride_elems != 3 && stride_elems != 4) || N < 2 || N > 894)
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_deposit_patches_host: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    const size_t pbytes = (size_t)N * N * N * stride_elems * (dtype == PSD_F32 ? 4 : 8);
+    CK(ctx->host_pos.ensure(pbytes));
+    CK(cudaMemcpyAsync(ctx->host_pos.p, pos_host, pbytes, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = psd_build_tets(ctx, ctx->host_pos.p, dtype, stride_elems, N, L, total_mass);
+    if (rc) return rc;
+    rc = psd_refine_patches(ctx, base_G, P, max_level, factor, rule, patches_out_host, cap, n_out, nullptr);
+    if (rc) return rc;
+    const size_t mbytes = sizeof(double) * (size_t)*n_out * P * P * P;
+    CK(ctx->host_grid.ensure(mbytes));
+    rc = psd_deposit_patches(ctx, patches_out_host, *n_out, P, base_G, ctx->host_grid.as<double>(), 0);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(mass_host, ctx->host_grid.p, mbytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PSD_OK;
+}
+
 int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
     if (!valid_ctx(ctx) || !out) return PSD_ERR_INVALID_ARG;
     CK(cudaSetDevice(ctx->device));

@@ -326,6 +326,53 @@ def test_host_buffer_entry_point(psd, ctx, oracle):
     assert_parity(ng, ora)
 
 
+def test_patches_host_buffer_entry_point(psd, ctx, oracle):
+    """psd_deposit_patches_host: positions from host memory, refinement + deposit, masses back to
+    host memory in one C-ABI call -- the same list and the same masses as the device calls."""
+    import torch
+    pos = crossing_field(16, 2.5, dtype="float32", stride=4, modes=40, kmax=4)
+    base_G, P, max_level, factor = 32, 16, 2, 1.5
+    ctx.psd_build_tets(to_dev(pos))
+    want_list = ctx.psd_refine_patches(base_G, P, max_level, factor)
+    cap = sum(((base_G << l) // P) ** 3 for l in range(max_level + 1))
+    hm = torch.full((cap, P, P, P), -1.0, dtype=torch.float64).pin_memory()
+    got_list = ctx.psd_deposit_patches_host(torch.from_numpy(pos).pin_memory(), base_G, P, max_level, factor, hm)
+    assert np.array_equal(got_list, want_list)
+    n = len(got_list)
+    ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, got_list)
+    assert_parity(hm.numpy()[:n], ora)
+    assert (hm.numpy()[n:] == -1.0).all()      # nothing written past the list
+    # pageable numpy buffers, and a buffer that is too small for the list
+    nm = np.zeros((cap, P, P, P))
+    assert np.array_equal(ctx.psd_deposit_patches_host(pos, base_G, P, max_level, factor, nm), want_list)
+    assert_parity(nm[:n], ora)
+    with pytest.raises(psd.PsdError) as e:
+        ctx.psd_deposit_patches_host(pos, base_G, P, max_level, factor, np.zeros((n - 1, P, P, P)))
+    assert e.value.code == 1
+
+
+def test_host_entry_points_validate_their_buffers(psd, ctx):
+    """The host entry points take raw addresses: dtype, size, contiguity and residency are checked
+    in the binding before the library writes G^3 (or n P^3) doubles through them."""
+    import torch
+    pos = crossing_field(6, 0.5, dtype="float32", stride=4)
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_uniform_host(pos, 16, np.zeros((16, 16, 16), dtype=np.float32))
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_uniform_host(pos, 16, np.zeros((16, 16, 15)))
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_uniform_host(pos, 16, np.zeros((16, 16, 32))[:, :, ::2])
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_uniform_host(pos, 16, torch.zeros((16, 16, 16), dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_uniform_host(pos[:, :, ::2][:, :, :3], 16, np.zeros((16, 16, 16)))
+    with pytest.raises(ValueError):
+        ctx.psd_deposit_patches_host(pos, 16, 8, 1, 2.0, np.zeros((4, 8, 8, 8), dtype=np.float32))
+    g = np.zeros((16, 16, 16))
+    ctx.psd_deposit_uniform_host(pos, 16, g)
+    assert_mass(g.sum())
+
+
 def test_runs_on_a_non_default_stream(psd, oracle):
     import torch
     pos = crossing_field(10, 1.0)
