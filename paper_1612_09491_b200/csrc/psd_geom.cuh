@@ -208,7 +208,7 @@ __device__ __forceinline__ double fast_rcp(double x) {
 template <int S>
 struct PolyBuf {
     double* p;
-    __device__ __forceinline__ double& at(int i, int c) { return p[(3 * i + c) * S]; }
+    __host__ __device__ __forceinline__ double& at(int i, int c) { return p[(3 * i + c) * S]; }
 };
 
 
@@ -231,7 +231,7 @@ __device__ __forceinline__ unsigned gather_nibble_bit(unsigned x, int k) {
     return (y | (y >> 12)) & 0x7fu;
 }
 
-__device__ __forceinline__ int slot_of(unsigned order, int i) { return (order >> (4 * i)) & 7; }
+__host__ __device__ __forceinline__ int slot_of(unsigned order, int i) { return (order >> (4 * i)) & 15; }
 __device__ __forceinline__ unsigned nib_mask(int n) { return n >= 8 ? 0xffffffffu : ((1u << (4 * n)) - 1u); }
 
 // The two edges where a convex polygon with inside-bits `mask` (bit i: vertex i inside, neither
@@ -329,7 +329,7 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
     const int m = __popc(mask);
     double pv, pw, ph;  // first inside vertex, relative to X_in
     {
-        const int se = rot & 7;
+        const int se = rot & 15;
         const double he = q.at(se, 0) - a, hc = q.at(sc, 0) - a;
         const double t = he * fast_rcp(he - hc);
         const double ev = q.at(se, 1), ew = q.at(se, 2);
@@ -340,7 +340,7 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
 #pragma unroll
     for (int j = 1; j < POLY_CAP; ++j) {  // the inside vertices after the first
         if (j >= m) break;
-        const int s = (rot >> (4 * j)) & 7;
+        const int s = (rot >> (4 * j)) & 15;
         const double cv = q.at(s, 1) - x0v, cw = q.at(s, 2) - x0w, ch = q.at(s, 0) - a;
         sum = fma(pv * cw - pw * cv, ph + ch, sum);
         pv = cv; pw = cw; ph = ch;
@@ -384,6 +384,35 @@ __device__ __forceinline__ unsigned tri_outcodes(PolyBuf<S> q, unsigned& all_in,
     return oc;
 }
 
+// Signed projected area A and first moment M1 = integral of u over the convex polygon
+// (order, n), fanned from its vertex 0; floor / ceil of its lowest / highest vertex.
+template <int S>
+__device__ __forceinline__ FaceClip poly_area_moment(PolyBuf<S> q, unsigned order, int n) {
+    FaceClip fc;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
+    if (n < 3) return fc;
+    const int s0 = slot_of(order, 0), s1 = slot_of(order, 1);
+    const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
+    double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
+    int ifl = min(__double2int_rd(u0), __double2int_rd(lu)), ice = max(__double2int_ru(u0), __double2int_ru(lu));
+    double A2 = 0.0, M6 = 0.0;
+#pragma unroll
+    for (int i = 2; i < POLY_CAP; ++i) {
+        if (i >= n) break;
+        const int s = slot_of(order, i);
+        const double cu = q.at(s, 0), cv = q.at(s, 1) - v0, cw = q.at(s, 2) - w0;
+        const double cr = lv * cw - lw * cv;
+        A2 += cr;
+        M6 = fma(cr, u0 + lu + cu, M6);
+        ifl = min(ifl, __double2int_rd(cu)); ice = max(ice, __double2int_ru(cu));
+        lu = cu; lv = cv; lw = cw;
+    }
+    fc.order = order; fc.n = n;
+    fc.A = 0.5 * A2; fc.M1 = M6 * (1.0 / 6.0);
+    fc.ifl = ifl; fc.ice = ice;
+    return fc;
+}
+
 template <int S, bool WALLS_UNROLLED>
 __device__ __forceinline__ FaceClip face_clip_oc(PolyBuf<S> q, unsigned oc, unsigned all_in, unsigned any_in);
 
@@ -415,28 +444,7 @@ __device__ __forceinline__ FaceClip face_clip_oc(PolyBuf<S> q, unsigned oc, unsi
             clip_wall<S, false>(q, r, wall);
         }
     }
-    if (r.n < 3) return fc;
-    // signed projected area A and first moment M1 = integral of u over Q, fan from vertex 0
-    const int s0 = slot_of(r.order, 0), s1 = slot_of(r.order, 1);
-    const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
-    double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
-    int ifl = min(__double2int_rd(u0), __double2int_rd(lu)), ice = max(__double2int_ru(u0), __double2int_ru(lu));
-    double A2 = 0.0, M6 = 0.0;
-#pragma unroll
-    for (int i = 2; i < POLY_CAP; ++i) {
-        if (i >= r.n) break;
-        const int s = slot_of(r.order, i);
-        const double cu = q.at(s, 0), cv = q.at(s, 1) - v0, cw = q.at(s, 2) - w0;
-        const double cr = lv * cw - lw * cv;
-        A2 += cr;
-        M6 = fma(cr, u0 + lu + cu, M6);
-        ifl = min(ifl, __double2int_rd(cu)); ice = max(ice, __double2int_ru(cu));
-        lu = cu; lv = cv; lw = cw;
-    }
-    fc.order = r.order; fc.n = r.n;
-    fc.A = 0.5 * A2; fc.M1 = M6 * (1.0 / 6.0);
-    fc.ifl = ifl; fc.ice = ice;
-    return fc;
+    return poly_area_moment<S>(q, r.order, r.n);
 }
 
 // Cells and planes of a clipped face over the run of cells c_lo..c_hi (cell c spans u in [c,c+1]).

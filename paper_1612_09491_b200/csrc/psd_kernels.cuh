@@ -6,6 +6,7 @@
 //   a7 patch path            the same kernels with Space::patch_mode = 1, k_patch_counts
 #pragma once
 #include "psd_geom.cuh"
+#include "psd_lbclip.cuh"
 
 namespace psd {
 
@@ -391,18 +392,24 @@ struct DepositArgs {
 };
 
 #ifndef DEP_MIN_CTAS
-#define DEP_MIN_CTAS 5
+#define DEP_MIN_CTAS 3
 #endif
 #ifndef DEP_WARPS_N
-#define DEP_WARPS_N 4
+#define DEP_WARPS_N 6
 #endif
 constexpr int DEP_WARPS = DEP_WARPS_N;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
-// [3*POLY_CAP][32], face rectangles [32] (u64), slot words [32] (u32), job queues (u32)
-constexpr int N_QUEUES = 3, QUEUE_CAP = 64;  // job queues by clip class, u32 descriptors
-constexpr int WARP_SCRATCH = (13 + 3 * POLY_CAP) * 32 + 32 + 16 + N_QUEUES * QUEUE_CAP / 2;
+// [3*LB_SLOTS][32], face rectangles [32] (u64), slot words [32] (u32)
+constexpr int WARP_SCRATCH = (13 + 3 * LB_SLOTS) * 32 + 32 + 16;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
+
+// The general convex clip (clip_wall) of one face job, for the jobs the straight-line clip
+// reports as ambiguous (lattice-aligned input): kept out of line, it runs rarely.
+__device__ __noinline__ FaceClip face_clip_general(double* lane_poly) {  // triangle in slots 0..2
+    PolyBuf<32> q{lane_poly};
+    return face_clip<32, false>(q);
+}
 
 __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile, int& level,
                                               int org[3], double*& out, long long str[3]) {
@@ -428,11 +435,12 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
 // memory.  Each warp takes 32 pairs at a time:
 //   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
 //            into the warp's slots; per face the rectangle of columns its projection meets.
-//   stage B  the face jobs (slot, face, column) of the 32 slots are numbered by a warp prefix
-//            sum of the rectangle sizes; lane = job computes its triangle's outcodes and queues
-//            the job by clip class (how many walls have a vertex beyond them).
-//   stage C  32 jobs of one queue at a time, lane = job: wall clip, trivial cells; then the
-//            cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
+//   stage B  the face jobs (slot, face, column) of the 32 slots, face by face, are numbered by a
+//            warp prefix sum of the rectangle sizes, 32 at a time with lane = job: the triangle
+//            against its column in straight-line code (tri_square_clip: parametric clip of the 3
+//            edges, corners by wall ids; no vertex list is edited, so the lanes do not diverge on
+//            the number of walls), projected area and moment, trivial cells.
+//   stage C  the cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
 //            integrals, shares added to the tile (a4-a6).
 // The tile is flushed to global memory with fp64 reductions at the end (a6).
 template <bool COUNT>
@@ -441,11 +449,15 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
-    double* wpoly = wtet + 13 * 32;                                                    // [24][32]
-    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * POLY_CAP * 32);  // [32]
+    double* wpoly = wtet + 13 * 32;                                                    // [3 * LB_SLOTS][32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [32]
     unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 32);                 // [32]
-    unsigned int* wq = wword + 32;                                                     // [N_QUEUES][QUEUE_CAP]
     PolyBuf<32> poly{wpoly + lane};
+    // slots 6..9 of the lane's polygon buffer hold the corners of the column's unit square: their
+    // (v, w) never change (the general clip may overwrite slot 6: restored before the next job)
+    poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; poly.at(7, 1) = 1.0; poly.at(7, 2) = 0.0;
+    poly.at(8, 1) = 1.0; poly.at(8, 2) = 1.0; poly.at(9, 1) = 0.0; poly.at(9, 2) = 1.0;
+    bool slot6_dirty = false;
 
     const Item item = A.items[blockIdx.x];
     int level, org[3];
@@ -576,34 +588,44 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 wrect[lane] = rect;
                 wword[lane] = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
-            // ---- stage C (a lambda: runs once per 32 queued jobs).  C1: lane = face job, wall clip
-            // (outcodes given), the polygon stays in the lane's buffer, trivial cells.  C2: the
+            // ---- stages B + C for 32 jobs (a lambda with a single call site: its code is large).
+            // B: lane = face job (slot, f, cv, cw): clip, area and moment, trivial cells.  C: the
             // cutting planes (polygon, a) of the 32 jobs, numbered by a warp prefix sum, lane = plane;
             // the kept part above the plane is integrated in closed form; +R to cell a, -R to a-1.
-            auto run_jobs = [&](const bool act, const unsigned int desc) {
+            auto run_jobs = [&](const bool act, const int slot, const int f, const int cv, const int cw) {
                 unsigned int f_order = 0, f_info = 0;
                 int f_afirst = 0, k = 0;
                 double f_w = 0.0;
                 if (act) {
-                    const int slot = desc & 31, f = (desc >> 5) & 3, cv = (desc >> 7) & 7, cw = (desc >> 10) & 7;
-                    const unsigned int oc = (desc >> 13) & 0xfffu;
+                    if (COUNT) cnt.jobs++;
                     const unsigned int word = wword[slot];
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-                    // the face triangle, column-local, into slots 0..2 of the lane's polygon buffer
+                    // the face triangle, column-local
                     const double* ts = wtet + slot;
                     const unsigned int fv = FACE_TABLE >> (6 * f);
                     const double ov = (double)cv, ow = (double)cw;
+                    double U[3], V[3], W[3];
 #pragma unroll
                     for (int i = 0; i < 3; ++i) {
                         const int vi = (fv >> (2 * i)) & 3;
-                        poly.at(i, 0) = ts[(3 * vi + ax) * 32];
-                        poly.at(i, 1) = ts[(3 * vi + av) * 32] - ov;
-                        poly.at(i, 2) = ts[(3 * vi + aw) * 32] - ow;
+                        U[i] = ts[(3 * vi + ax) * 32];
+                        V[i] = ts[(3 * vi + av) * 32] - ov;
+                        W[i] = ts[(3 * vi + aw) * 32] - ow;
                     }
                     f_w = ts[12 * 32];
-                    const unsigned int all_in = oc & (oc >> 4) & (oc >> 8) & 15u;
-                    const FaceClip fc = face_clip_oc<32, false>(poly, oc, all_in, 15u);
+                    if (slot6_dirty) { poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; slot6_dirty = false; }
+                    const LBResult lb = tri_square_clip<32>(poly, U, V, W);
+                    FaceClip fc;
+                    if (lb.amb) {
+#pragma unroll
+                        for (int i = 0; i < 3; ++i) { poly.at(i, 0) = U[i]; poly.at(i, 1) = V[i]; poly.at(i, 2) = W[i]; }
+                        fc = face_clip_general(wpoly + lane);
+                        slot6_dirty = true;
+                    } else {
+                        fc = poly_area_moment<32>(poly, lb.order, lb.n);
+                        if (lb.sign < 0) f_w = -f_w;  // clockwise triangle: the polygon is its mirror image
+                    }
                     if (fc.n >= 3 && fc.ice > c_lo) {
                         if (COUNT) cnt.face_clips++;
                         const FaceRun fr = face_run(fc, c_lo, c_hi);
@@ -678,32 +700,14 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 }
                 __syncwarp();
             };
-            // ---- stage B: the face jobs (slot, face, column) of the 32 slots, face by face, numbered
-            // by a warp prefix sum of the rectangle sizes; lane = job computes the outcodes of its
-            // triangle against its column and queues the job by CLIP CLASS (walls with a vertex
-            // beyond them: <= 2, 3, 4), so that the 32 jobs stage C takes from one queue clip about
-            // the same number of walls.  A queue runs as soon as it holds 32 jobs; the rest at the end.
-            // One loop with a single call site of stage C (its code is large): drain a queue that
-            // holds 32 jobs, else generate the next 32 jobs, at the end drain what is left.
+            // ---- the face jobs (slot, face, column) of the 32 slots, face by face, numbered by a warp
+            // prefix sum of the rectangle sizes; one loop with a single call site of run_jobs
             __syncwarp();
-            int qn0 = 0, qn1 = 0, qn2 = 0;  // N_QUEUES = 3 queue lengths (warp-uniform)
             int f = -1, jb = 0, total = 0, pre = 0;
-            bool flushing = false;
 #pragma unroll 1
             for (;;) {
-                const int thr = flushing ? 1 : 32;
-                const int c = qn0 >= thr ? 0 : (qn1 >= thr ? 1 : (qn2 >= thr ? 2 : -1));
-                if (c >= 0) {
-                    const int have_n = c == 0 ? qn0 : (c == 1 ? qn1 : qn2);
-                    const int take = min(have_n, 32), left = have_n - take;
-                    if (c == 0) qn0 = left; else if (c == 1) qn1 = left; else qn2 = left;
-                    __syncwarp();
-                    run_jobs(lane < take, lane < take ? wq[c * QUEUE_CAP + left + lane] : 0u);
-                    continue;
-                }
-                if (flushing) break;
                 if (jb >= total) {  // next face: exclusive prefix of its job counts over the 32 slots
-                    if (++f == 4) { flushing = true; continue; }
+                    if (++f == 4) break;
                     const int njobs = (cnts >> (8 * f)) & 255;
                     pre = njobs;
                     for (int o = 1; o < 32; o <<= 1) {
@@ -724,11 +728,10 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     if (probe <= job) slot += step;
                 }
                 const int spre = __shfl_sync(0xffffffffu, pre, slot);
-                unsigned int desc = 0;
-                int cls = -1;
-                if (job < total) {
+                int cv = 0, cw = 0;
+                const bool act = job < total;
+                if (act) {
                     // decode (slot, column)
-                    const unsigned int word = wword[slot];
                     const int local = job - spre;
                     const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
                     const int nw = ((r16 >> 9) & 7) + 1;
@@ -736,34 +739,9 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     // (local * ceil(256 / nw)) >> 8 is exact there; the table holds ceil(256/nw) - 1
                     const int inv = (int)((0x1f242a333f557fffull >> (8 * (nw - 1))) & 255ull) + 1;
                     const int lq = (local * inv) >> 8;
-                    const int cv = (r16 & 7) + lq, cw = ((r16 >> 6) & 7) + (local - lq * nw);
-                    const int ax = word & 3;
-                    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-                    const double* ts = wtet + slot;
-                    const unsigned int fv = FACE_TABLE >> (6 * f);
-                    const double ov = (double)cv, ow = (double)cw;
-                    unsigned int oc = 0, all_in = 15u;
-#pragma unroll
-                    for (int i = 0; i < 3; ++i) {
-                        const int vi = (fv >> (2 * i)) & 3;
-                        const double v = ts[(3 * vi + av) * 32] - ov, w = ts[(3 * vi + aw) * 32] - ow;
-                        const unsigned int o = (unsigned)(v >= 0.0) | (unsigned)(v <= 1.0) << 1 |
-                                               (unsigned)(w >= 0.0) << 2 | (unsigned)(w <= 1.0) << 3;
-                        oc |= o << (4 * i);
-                        all_in &= o;
-                    }
-                    if (COUNT) cnt.jobs++;
-                    const int pc = __popc(all_in ^ 15u);
-                    cls = pc <= 2 ? 0 : (pc == 3 ? 1 : 2);
-                    desc = (unsigned)slot | (unsigned)f << 5 | (unsigned)cv << 7 | (unsigned)cw << 10 | oc << 13;
+                    cv = (r16 & 7) + lq; cw = ((r16 >> 6) & 7) + (local - lq * nw);
                 }
-                const unsigned int lt = (1u << lane) - 1u;
-                const unsigned int m0 = __ballot_sync(0xffffffffu, cls == 0), m1 = __ballot_sync(0xffffffffu, cls == 1);
-                const unsigned int m2 = __ballot_sync(0xffffffffu, cls == 2);
-                if (cls == 0) wq[0 * QUEUE_CAP + qn0 + __popc(m0 & lt)] = desc;
-                if (cls == 1) wq[1 * QUEUE_CAP + qn1 + __popc(m1 & lt)] = desc;
-                if (cls == 2) wq[2 * QUEUE_CAP + qn2 + __popc(m2 & lt)] = desc;
-                qn0 += __popc(m0); qn1 += __popc(m1); qn2 += __popc(m2);
+                run_jobs(act, slot, f, cv, cw);
             }
         }
     }
