@@ -168,6 +168,17 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         A.weight_mode = ctx->weight_mode;
         A.chord_axis = ctx->chord_axis;
         A.stats = ctx->stats.as<unsigned long long>();
+        {
+            // fixed-point unit of the tile accumulators: a cell of one work item receives at most
+            // chunk x (mass of a tet, or one cell volume in signed-volume mode); 2^62 / that, as a
+            // power of two
+            const double unit = ctx->weight_mode == 0 ? std::fabs(A.mass_per_tet) : 1.0;
+            int eu = 0, ec = 0;
+            if (unit > 0.0 && std::isfinite(unit)) std::frexp(unit, &eu);   // unit < 2^eu
+            std::frexp((double)ctx->chunk, &ec);                            // chunk < 2^ec
+            A.acc_scale = std::ldexp(1.0, 61 - eu - ec);
+            A.acc_inv_scale = std::ldexp(1.0, -(61 - eu - ec));
+        }
         if (n_slabs > 1) {
             // one launch per slab of x-tiles (items are in tile order); the finished slab of the grid
             // goes to the host on the copy stream while the next slabs are deposited
@@ -235,6 +246,7 @@ int run_direct(psd_ctx* ctx, Space space) {
     A.weight_mode = ctx->weight_mode;
     A.chord_axis = ctx->chord_axis;
     A.stats = ctx->stats.as<unsigned long long>();
+    A.acc_scale = A.acc_inv_scale = 1.0;  // the direct path adds to global memory in fp64
     const unsigned int grid = (unsigned int)((ntet + 127) / 128);
     if (ctx->counters) k_deposit_direct<true><<<grid, 128, 0, st>>>(A);
     else k_deposit_direct<false><<<grid, 128, 0, st>>>(A);

@@ -389,7 +389,58 @@ struct DepositArgs {
     int weight_mode;  // 0 mass, 1 signed volume
     int chord_axis;   // -1 adaptive, else 0..2
     unsigned long long* stats;
+    double acc_scale, acc_inv_scale;  // fixed-point tile accumulators (PSD_ACC_FIXED): a power of two and its inverse
 };
+
+
+// a6, the tile accumulator.  Shared memory has no native 64-bit atomic add on sm_100a (fp64 and
+// u64 atomicAdd both compile to an ATOMS.CAST.SPIN.64 compare-and-swap loop); only the 32-bit
+// integer ATOMS.ADD is native.  With PSD_ACC_FIXED a cell is a 64-bit two's-complement fixed-point
+// number (unit 1 / acc_scale, a power of two, so that the scaling is exact) held in two 32-bit
+// limbs: the low limb is added with one native atomic that returns the old value, the carry out
+// of it goes with the high limb in a second one.  Integer addition commutes and every carry is
+// added exactly once, so the two limbs end up exact whatever the interleaving; sums wrap modulo
+// 2^64, which is harmless as long as the final value of the cell fits (it is bounded by the
+// chunk size times the mass of a tet, and acc_scale is chosen from that).
+#ifndef PSD_ACC_FIXED
+#define PSD_ACC_FIXED 1
+#endif
+struct TileShare {
+#if PSD_ACC_FIXED
+    unsigned int lo, hi;
+#else
+    double x;
+#endif
+};
+__device__ __forceinline__ TileShare tile_share(double x, double scale) {
+    TileShare q;
+#if PSD_ACC_FIXED
+    double y = x * scale;
+    if (fabs(y) >= 0x1p62) y -= 0x1p64 * rint(y * 0x1p-64);  // sliver tets: reduce modulo 2^64 (exact)
+    const long long v = __double2ll_rn(y);
+    q.lo = (unsigned int)v; q.hi = (unsigned int)(v >> 32);
+#else
+    q.x = x;
+#endif
+    return q;
+}
+__device__ __forceinline__ void tile_add(double* cell, TileShare q) {
+#if PSD_ACC_FIXED
+    unsigned int* a = reinterpret_cast<unsigned int*>(cell);
+    const unsigned int old = atomicAdd(a, q.lo);
+    atomicAdd(a + 1, q.hi + (unsigned int)(old + q.lo < old));
+#else
+    atomicAdd(cell, q.x);
+#endif
+}
+__device__ __forceinline__ double tile_value(const double* cell, double inv_scale) {
+#if PSD_ACC_FIXED
+    const unsigned int* a = reinterpret_cast<const unsigned int*>(cell);
+    return (double)(long long)(((unsigned long long)a[1] << 32) | a[0]) * inv_scale;
+#else
+    return *cell;
+#endif
+}
 
 #ifndef DEP_MIN_CTAS
 #define DEP_MIN_CTAS 3
@@ -542,13 +593,13 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                             c[x] = __double2int_rd(cen) - (org[x] + m[x] * Gl);
                             in = in && c[x] >= 0 && c[x] < TILE;
                         }
-                        if (in) atomicAdd(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], A.mass_per_tet);
+                        if (in) tile_add(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], tile_share(A.mass_per_tet, A.acc_scale));
                     }
                 } else if (t.lo[0] == t.hi[0] && t.lo[1] == t.hi[1] && t.lo[2] == t.hi[2]) {
                     // a4, tet inside one cell ("trivial cases"): the whole tet goes
                     // to that cell -- m, or its signed volume det/6 in signed-volume mode
-                    atomicAdd(&acc[(lo[0] * TILE + lo[1]) * TILE + lo[2]],
-                              A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0));
+                    tile_add(&acc[(lo[0] * TILE + lo[1]) * TILE + lo[2]],
+                             tile_share(A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0), A.acc_scale));
                 } else {
                     // per vertex: floor / ceil of (v, w) and ceil of u, read back through the
                     // runtime axis (the lane's own stores above); the faces' rectangles are then
@@ -640,18 +691,19 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                             const int full_hi = min(fr.t_hi, fc.ifl - 1);  // cells entirely below Q
                             const double wA = f_w * fc.A;
                             if (wA != 0.0) {
+                                const TileShare qA = tile_share(wA, A.acc_scale);
 #pragma unroll
                                 for (int cc = 0; cc < TILE; ++cc) {
                                     const int c = c_lo + cc;
                                     if (c > full_hi) break;
-                                    atomicAdd(acc + colofs + c * su, wA);
+                                    tile_add(acc + colofs + c * su, qA);
                                     if (COUNT) cnt.cells++;
                                 }
                             }
                             if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {  // the cell holding umin
                                 const double D = fma(-(double)fc.ifl, fc.A, fc.M1);
                                 if (D != 0.0) {
-                                    atomicAdd(acc + colofs + fc.ifl * su, f_w * D);
+                                    tile_add(acc + colofs + fc.ifl * su, tile_share(f_w * D, A.acc_scale));
                                     if (COUNT) cnt.cells++;
                                 }
                             }
@@ -693,8 +745,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         const double R = plane_integral6<32>(qs, s_order, n, (double)a) * (1.0 / 6.0) * s_w;
                         if (COUNT) cnt.plane_evals++;
                         if (R != 0.0) {
-                            if (a <= c_hi) { atomicAdd(acc + colofs + a * su, R); if (COUNT) cnt.cells++; }
-                            if (a - 1 >= c_lo) { atomicAdd(acc + colofs + (a - 1) * su, -R); if (COUNT) cnt.cells++; }
+                            if (a <= c_hi) { tile_add(acc + colofs + a * su, tile_share(R, A.acc_scale)); if (COUNT) cnt.cells++; }
+                            if (a - 1 >= c_lo) { tile_add(acc + colofs + (a - 1) * su, tile_share(-R, A.acc_scale)); if (COUNT) cnt.cells++; }
                         }
                     }
                 }
@@ -748,7 +800,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
     __syncthreads();
     // ---- a6: flush the tile with fp64 reductions (other work items may hold the same tile)
     for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) {
-        double v = acc[i];
+        const double v = tile_value(acc + i, A.acc_inv_scale);
         if (v != 0.0) {
             int cz = i & 7, cy = (i >> 3) & 7, cx = i >> 6;
             atomicAdd(out + cx * str[0] + cy * str[1] + cz, v);
