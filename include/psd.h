@@ -72,10 +72,17 @@ enum {
                                 shorter than L/2 (minimum-image unwrap) and meets at most 64
                                 patch positions per axis, else PSD_ERR_UNWRAP.                */
     ,
-    PSD_OPT_CLASS_SMALL_CELLS = 6 /* a3 size classes of the binned path: a (tet, tile) pair whose
+    PSD_OPT_CLASS_SMALL_CELLS = 6, /* a3 size classes of the binned path: a (tet, tile) pair whose
                                 cell range covers at most this many cells of the tile is class
                                 "small", else "large"; a power of two in [1, 512] (default 8) so
                                 that the classes are unions of the census buckets hist_pair[b] */
+    PSD_OPT_PATCH_RESTRICT = 7  /* psd_deposit_patches, PAPER.md:193 (coarser representations of the
+                                internal nodes).  1 (default): a listed patch whose 8 children are
+                                all listed too is not deposited into; it is filled afterwards by
+                                summing the 2x2x2 cells of its children, finest level first (the
+                                children tile it, so this is the same mass up to rounding).
+                                0: every listed patch is deposited into directly (Q13).
+                                Ignored (as 0) when accumulate = 1 or P is odd.                */
 };
 
 #define PSD_SUBBLOCK_UNIT (1u << 20)
@@ -108,6 +115,7 @@ typedef struct {
     int64_t n_face_clips;   /* jobs whose clipped polygon is non-empty and reaches the run */
     int64_t n_plane_evals;  /* closed-form lattice-plane integrals of a face polygon     */
     int64_t n_cells_written;/* per-face cell shares added to accumulators                */
+    int64_t n_restricted_patches; /* psd_deposit_patches: patches filled from their children     */
     /* device pointer to the per-(tile, size class) pair counts of the last binned deposit
        (2 * n_tiles uint32, see psd_get_tile_class_counts) */
     const uint32_t* tile_counts_dev;

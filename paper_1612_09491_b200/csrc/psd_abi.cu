@@ -41,11 +41,11 @@ struct psd_ctx {
     Particles part{};
     bool built = false;
     double total_mass = 0.0;
-    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0;
+    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1;
     long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 1024;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
-        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid;
+        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families;
     unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
     psd_stats last{};
     bool stats_pending = false;
@@ -300,7 +300,7 @@ void psd_destroy(psd_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->tile_counts, &ctx->cursors, &ctx->tile_offsets, &ctx->item_offsets, &ctx->items,
                       &ctx->pair_ids, &ctx->part_pairs, &ctx->part_items, &ctx->totals, &ctx->stats, &ctx->hist,
-                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid};
+                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families};
     for (DevBuf* b : bufs) b->release();
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 6; ++i)
@@ -406,20 +406,60 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
         long long np = ((long long)base_G << l) / P;
         total += np * np * np;
     }
-    std::vector<int> lookup((size_t)total, -1);
-    for (int64_t q = 0; q < n_patch; ++q) {
-        const psd_patch& pp = patches_host[q];
-        long long np = ((long long)base_G << pp.level) / P;
-        long long idx = s.lookup_off[pp.level] + ((long long)pp.ox * np + pp.oy) * np + pp.oz;
-        if (lookup[(size_t)idx] != -1) return fail(ctx, PSD_ERR_INVALID_ARG, "duplicate patch in list");
-        lookup[(size_t)idx] = (int)q;
+    std::vector<int> lookup;
+    std::vector<int> fam;                       // per refined patch: its index, then its 8 children
+    std::vector<long long> fam_level_begin;     // first family of each level (families sorted by level)
+    try {
+        lookup.assign((size_t)total, -1);
+        for (int64_t q = 0; q < n_patch; ++q) {
+            const psd_patch& pp = patches_host[q];
+            long long np = ((long long)base_G << pp.level) / P;
+            long long idx = s.lookup_off[pp.level] + ((long long)pp.ox * np + pp.oy) * np + pp.oz;
+            if (lookup[(size_t)idx] != -1) return fail(ctx, PSD_ERR_INVALID_ARG, "duplicate patch in list");
+            lookup[(size_t)idx] = (int)q;
+        }
+        // a patch whose 8 children are all listed is filled by restriction, not deposited
+        // into (PSD_OPT_PATCH_RESTRICT; not when accumulating: the children then hold old + new mass)
+        if (ctx->patch_restrict && !accumulate && P % 2 == 0) {
+            fam_level_begin.assign((size_t)max_level + 2, 0);
+            for (int l = 0; l < max_level; ++l) {
+                fam_level_begin[(size_t)l] = (long long)fam.size() / 9;
+                const long long npc = ((long long)base_G << (l + 1)) / P;
+                for (int64_t q = 0; q < n_patch; ++q) {
+                    const psd_patch& pp = patches_host[q];
+                    if (pp.level != l) continue;
+                    int ch[8];
+                    bool all = true;
+                    for (int d = 0; d < 8 && all; ++d) {
+                        const long long cx = 2ll * pp.ox + (d & 1), cy = 2ll * pp.oy + ((d >> 1) & 1), cz = 2ll * pp.oz + (d >> 2);
+                        ch[d] = lookup[(size_t)(s.lookup_off[l + 1] + (cx * npc + cy) * npc + cz)];
+                        all = ch[d] >= 0;
+                    }
+                    if (!all) continue;
+                    fam.push_back((int)q);
+                    for (int d = 0; d < 8; ++d) fam.push_back(ch[d]);
+                }
+            }
+            fam_level_begin[(size_t)max_level] = fam_level_begin[(size_t)max_level + 1] = (long long)fam.size() / 9;
+            // the deposit kernels find patches through `lookup`: refined ones are taken out of it
+            for (size_t i = 0; i < fam.size(); i += 9) {
+                const psd_patch& pp = patches_host[fam[i]];
+                long long np = ((long long)base_G << pp.level) / P;
+                lookup[(size_t)(s.lookup_off[pp.level] + ((long long)pp.ox * np + pp.oy) * np + pp.oz)] = -1;
+            }
+        }
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, PSD_ERR_OOM, "psd_deposit_patches: host allocation failed");
     }
     CK(ctx->lookup.ensure(sizeof(int) * (size_t)total));
     CK(ctx->patches.ensure(sizeof(PatchDev) * (size_t)n_patch));
+    if (!fam.empty()) CK(ctx->families.ensure(sizeof(int) * fam.size()));
     // pageable host memory: these copies complete before return, so the caller's list can go away
     CK(cudaMemcpyAsync(ctx->lookup.p, lookup.data(), sizeof(int) * (size_t)total, cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaMemcpyAsync(ctx->patches.p, patches_host, sizeof(PatchDev) * (size_t)n_patch, cudaMemcpyHostToDevice,
                        ctx->stream));
+    if (!fam.empty())
+        CK(cudaMemcpyAsync(ctx->families.p, fam.data(), sizeof(int) * fam.size(), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     s.lookup = ctx->lookup.as<int>();
     s.patches = ctx->patches.as<PatchDev>();
@@ -428,8 +468,22 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
     std::memset(&ctx->last, 0, sizeof(ctx->last));
     ctx->last.n_tets = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;
     ctx->last.n_nonfinite = nf;
-    return run_binned(ctx, s, (long long)n_patch * s.tp * s.tp * s.tp);
+    int rc = run_binned(ctx, s, (long long)n_patch * s.tp * s.tp * s.tp);
+    if (rc) return rc;
+    // restriction, finest refined level first (a parent's children may be refined themselves)
+    for (int l = max_level - 1; l >= 0 && !fam.empty(); --l) {
+        const long long b = fam_level_begin[(size_t)l], e = fam_level_begin[(size_t)l + 1];
+        if (e <= b) continue;
+        const long long threads = (e - b) * (long long)P * P * P;
+        k_restrict<<<(unsigned int)((threads + 255) / 256), 256, 0, ctx->stream>>>(ctx->families.as<int>() + b * 9, e - b, P,
+                                                                                   mass_dev);
+        ctx->launches += 1;
+    }
+    CK(cudaGetLastError());
+    ctx->last.n_restricted_patches = (int64_t)(fam.size() / 9);
+    return PSD_OK;
 }
+
 
 int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double factor, int rule,
                        psd_patch* out_host, int64_t cap, int64_t* n_out, uint64_t* counts_host) {
@@ -668,6 +722,9 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
             if (iv < 1 || iv > TILE_CELLS || (iv & (iv - 1)))
                 return fail(ctx, PSD_ERR_INVALID_ARG, "class threshold must be a power of two in [1, 512]");
             ctx->class_small = iv; return PSD_OK;
+        case PSD_OPT_PATCH_RESTRICT:
+            if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "patch restriction must be 0 or 1");
+            ctx->patch_restrict = iv; return PSD_OK;
         case PSD_OPT_REFINE_SUBBLOCK:
             if (iv < 0 || iv > 64) return fail(ctx, PSD_ERR_INVALID_ARG, "sub-block edge must be 0 (off) or 1..64 cells");
             ctx->refine_subblock = iv; return PSD_OK;

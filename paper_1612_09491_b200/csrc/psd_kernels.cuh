@@ -1015,6 +1015,34 @@ __global__ void __launch_bounds__(256) k_patch_counts(Particles p, int base_G, i
     }
 }
 
+// a7 / PAPER.md:193 ("generating coarser representations for the internal nodes"): a patch all of
+// whose 8 children are listed is not deposited into; each of its cells is the sum of the 2x2x2
+// cells of the children that cover it (exact: the children tile the parent).  One thread per parent
+// cell; `fam` holds, per refined patch, its own index followed by its 8 children's indices, child
+// d = dx + 2 dy + 4 dz at position (2 ox + dx, 2 oy + dy, 2 oz + dz).  Run finest level first.
+__global__ void __launch_bounds__(256) k_restrict(const int* fam, long long n_fam, int P, double* mass) {
+    const long long P3 = (long long)P * P * P;
+    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= n_fam * P3) return;
+    const long long q = t / P3;
+    const int cell = (int)(t - q * P3);
+    const int z = cell % P, y = (cell / P) % P, x = cell / (P * P);
+    const int h = P / 2;
+    const int dx = x >= h, dy = y >= h, dz = z >= h;
+    const int* f = fam + q * 9;
+    const double* c = mass + (long long)f[1 + dx + 2 * dy + 4 * dz] * P3;
+    const int cx = 2 * (x - dx * h), cy = 2 * (y - dy * h), cz = 2 * (z - dz * h);
+    double sum = 0.0;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            const double* row = c + ((long long)(cx + a) * P + (cy + b)) * P + cz;
+            sum += row[0] + row[1];
+        }
+    mass[(long long)f[0] * P3 + cell] = sum;
+}
+
 // a7: the memory-lean census.  One warp per sub-block of B^3 Lagrangian cells:
 // the lanes stride over its (B+1)^3 particles (unwrapped to the minimum image of the first one)
 // for the bounding box, then over the candidate patch positions the box meets; each receives

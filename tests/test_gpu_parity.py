@@ -278,6 +278,48 @@ def test_patch_list_subset_and_order_independence(psd, ctx, oracle):
 
 
 # ------------------------------------------------------------------ boundary behaviour
+def test_patch_restriction_fills_refined_parents_from_their_children(psd, ctx, oracle):
+    """PAPER.md:193 / PSD_OPT_PATCH_RESTRICT: a patch whose 8 children are all listed is not deposited
+    into but summed from them.  Same masses as the direct deposit and as the oracle; a parent with
+    only some children listed is deposited directly; accumulate = 1 turns the restriction off."""
+    pos = crossing_field(16, 2.5, dtype="float32", stride=4, modes=40, kmax=4)
+    base_G, P, max_level, factor = 32, 16, 2, 1.5
+    ctx.psd_build_tets(to_dev(pos))
+    patches = ctx.psd_refine_patches(base_G, P, max_level, factor)
+    # plus one level-1 patch family made incomplete: drop one child of a refined level-0 patch
+    lv1 = np.nonzero(patches[:, 0] == 1)[0]
+    incomplete = np.delete(patches, lv1[-1], axis=0)
+    for plist in (patches, incomplete):
+        ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, plist)
+        ctx.psd_set_option(psd.OPT_PATCH_RESTRICT, 1)
+        m1 = ctx.psd_deposit_patches(plist, P, base_G).cpu().numpy()
+        n_restricted = ctx.psd_get_stats().n_restricted_patches
+        n_pairs_restricted = ctx.psd_get_stats().n_pairs
+        ctx.psd_set_option(psd.OPT_PATCH_RESTRICT, 0)
+        m0 = ctx.psd_deposit_patches(plist, P, base_G).cpu().numpy()
+        assert ctx.psd_get_stats().n_restricted_patches == 0
+        assert ctx.psd_get_stats().n_pairs > n_pairs_restricted      # fewer (tet, tile) pairs to deposit
+        assert n_restricted > 0
+        assert_parity(m1, ora, what="restricted")
+        assert_parity(m0, ora, what="direct")
+        assert np.allclose(m1, m0, rtol=1e-9, atol=1e-9 * ora.max())
+    # the number of patches filled by restriction = those with all 8 children in the list
+    def n_refined(plist):
+        have = {tuple(r) for r in plist.tolist()}
+        return sum(all((l + 1, 2 * a + (d & 1), 2 * b + ((d >> 1) & 1), 2 * c + (d >> 2)) in have for d in range(8))
+                   for l, a, b, c in plist.tolist())
+    ctx.psd_set_option(psd.OPT_PATCH_RESTRICT, 1)
+    for plist in (patches, incomplete):
+        ctx.psd_deposit_patches(plist, P, base_G)
+        assert ctx.psd_get_stats().n_restricted_patches == n_refined(plist)
+    assert n_refined(incomplete) < n_refined(patches)
+    # accumulate: direct deposit everywhere, twice the mass
+    m = ctx.psd_deposit_patches(patches, P, base_G)
+    m = ctx.psd_deposit_patches(patches, P, base_G, m, accumulate=True).cpu().numpy()
+    assert ctx.psd_get_stats().n_restricted_patches == 0
+    assert_parity(0.5 * m, oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches), what="accumulated")
+
+
 def test_error_codes(psd, ctx):
     import torch
     with pytest.raises(psd.PsdError) as e:
