@@ -465,6 +465,252 @@ int psdo_census(const void *pos, int dtype, int stride, int N, double L, int G, 
     return 0;
 }
 
+/* ---- O5 at full size: the same census, over Lagrangian slabs in parallel (per-thread
+ * counters, summed at the end: integer work, order free), split by the a3 size class of the
+ * pair (cells of the tet's range inside the tile <= small_max: "small", else "large"), and
+ * optionally restricted to a window of tiles win_lo[x] <= t < win_lo[x] + win_n[x] (wrapped
+ * tile coordinates; counts_small / counts_large are then dense over the window, hist_pair
+ * and n_pairs cover the window's pairs only; hist_tet and the other scalars all tets).
+ * Pinned against psdo_census (tests/test_oracle_deposit.py).                              */
+int psdo_census_classes(const void *pos, int dtype, int stride, int N, double L, int G, int tile,
+                        int64_t small_max, const int64_t *win_lo, const int64_t *win_n,
+                        uint32_t *counts_small, uint32_t *counts_large, uint64_t *hist_tet,
+                        uint64_t *hist_pair, int64_t *out_scalars) {
+    if (N < 2 || G < 1 || tile < 1 || G % tile) return 1;
+    particles_t p = {pos, dtype, stride, N, L};
+    const REAL scale = (REAL)G / (REAL)L;
+    const int64_t nt = G / tile;
+    int64_t wlo[3] = {0, 0, 0}, wn[3] = {nt, nt, nt};
+    if (win_lo && win_n)
+        for (int x = 0; x < 3; ++x) {
+            wlo[x] = win_lo[x]; wn[x] = win_n[x];
+            if (wn[x] < 1 || wn[x] > nt) return 1;
+        }
+    const size_t nout = (size_t)(wn[0] * wn[1] * wn[2]);
+    memset(counts_small, 0, sizeof(uint32_t) * nout);
+    memset(counts_large, 0, sizeof(uint32_t) * nout);
+    memset(hist_tet, 0, sizeof(uint64_t) * 64);
+    memset(hist_pair, 0, sizeof(uint64_t) * 64);
+    int64_t n_pairs = 0, sum_cells = 0, max_cells = 0, n_inv = 0;
+    int failed = 0;
+#pragma omp parallel
+    {
+        uint32_t *cs = (uint32_t *)calloc(nout, sizeof(uint32_t));
+        uint32_t *cl = (uint32_t *)calloc(nout, sizeof(uint32_t));
+        int64_t *cnt[3];
+        for (int x = 0; x < 3; ++x) cnt[x] = (int64_t *)calloc((size_t)nt, sizeof(int64_t));
+        uint64_t ht[64], hp[64];
+        memset(ht, 0, sizeof ht);
+        memset(hp, 0, sizeof hp);
+        int64_t t_pairs = 0, t_sum = 0, t_max = 0, t_inv = 0;
+        int ok = cs && cl && cnt[0] && cnt[1] && cnt[2];
+        if (!ok) {
+#pragma omp atomic write
+            failed = 1;
+        }
+#pragma omp for schedule(dynamic, 1)
+        for (int i = 0; i < N; ++i) {
+            if (!ok) continue;
+            for (int j = 0; j < N; ++j)
+                for (int k = 0; k < N; ++k) {
+                    REAL P[8][3];
+                    cell_corners(&p, i, j, k, P);
+                    for (int t = 0; t < 6; ++t) {
+                        tet_t tet;
+                        make_tet(P, t, scale, &tet);
+                        if (tet.det < 0) ++t_inv;
+                        int64_t ncell = 1;
+                        for (int x = 0; x < 3; ++x) ncell *= tet.hi[x] - tet.lo[x] + 1;
+                        t_sum += ncell;
+                        if (ncell > t_max) t_max = ncell;
+                        ht[bit_width_u64((uint64_t)(ncell - 1))]++;
+                        for (int x = 0; x < 3; ++x)
+                            for (int64_t c = tet.lo[x]; c <= tet.hi[x]; ++c) cnt[x][wrap(c, G) / tile]++;
+                        /* the distinct tiles per axis: those of the cells of the range */
+                        for (int64_t cx = tet.lo[0]; cx <= tet.hi[0]; ++cx) {
+                            int64_t tx = wrap(cx, G) / tile;
+                            if (cnt[0][tx] <= 0) continue; /* already visited (marked below) */
+                            int64_t nx = cnt[0][tx];
+                            cnt[0][tx] = -nx;
+                            int64_t rx = wrap(tx - wlo[0], nt);
+                            if (rx >= wn[0]) continue;
+                            for (int64_t cy = tet.lo[1]; cy <= tet.hi[1]; ++cy) {
+                                int64_t ty = wrap(cy, G) / tile;
+                                if (cnt[1][ty] <= 0) continue;
+                                int64_t ny = cnt[1][ty];
+                                cnt[1][ty] = -ny;
+                                int64_t ry = wrap(ty - wlo[1], nt);
+                                if (ry >= wn[1]) continue;
+                                for (int64_t cz = tet.lo[2]; cz <= tet.hi[2]; ++cz) {
+                                    int64_t tz = wrap(cz, G) / tile;
+                                    if (cnt[2][tz] <= 0) continue;
+                                    int64_t nz = cnt[2][tz];
+                                    cnt[2][tz] = -nz;
+                                    int64_t rz = wrap(tz - wlo[2], nt);
+                                    if (rz >= wn[2]) continue;
+                                    uint64_t inside = (uint64_t)(nx * ny * nz);
+                                    size_t o = (size_t)((rx * wn[1] + ry) * wn[2] + rz);
+                                    if ((int64_t)inside <= small_max) cs[o]++; else cl[o]++;
+                                    ++t_pairs;
+                                    hp[bit_width_u64(inside - 1)]++;
+                                }
+                                for (int64_t cz = tet.lo[2]; cz <= tet.hi[2]; ++cz) { /* unmark z */
+                                    int64_t tz = wrap(cz, G) / tile;
+                                    if (cnt[2][tz] < 0) cnt[2][tz] = -cnt[2][tz];
+                                }
+                            }
+                            for (int64_t cy = tet.lo[1]; cy <= tet.hi[1]; ++cy) { /* unmark y */
+                                int64_t ty = wrap(cy, G) / tile;
+                                if (cnt[1][ty] < 0) cnt[1][ty] = -cnt[1][ty];
+                            }
+                        }
+                        for (int x = 0; x < 3; ++x) /* clear the touched entries */
+                            for (int64_t c = tet.lo[x]; c <= tet.hi[x]; ++c) cnt[x][wrap(c, G) / tile] = 0;
+                    }
+                }
+        }
+#pragma omp critical
+        {
+            if (ok) {
+                for (size_t o = 0; o < nout; ++o) { counts_small[o] += cs[o]; counts_large[o] += cl[o]; }
+                for (int b = 0; b < 64; ++b) { hist_tet[b] += ht[b]; hist_pair[b] += hp[b]; }
+                n_pairs += t_pairs; sum_cells += t_sum; n_inv += t_inv;
+                if (t_max > max_cells) max_cells = t_max;
+            }
+        }
+        free(cs); free(cl);
+        for (int x = 0; x < 3; ++x) free(cnt[x]);
+    }
+    if (failed) return 2;
+    out_scalars[0] = (int64_t)6 * N * N * N;
+    out_scalars[1] = n_pairs;
+    out_scalars[2] = sum_cells;
+    out_scalars[3] = max_cells;
+    out_scalars[4] = n_inv;
+    return 0;
+}
+
+/* Deposit into K windows of the grid in one pass over the tets (the windows of psdo_deposit_window;
+ * out holds them one after the other, window w has win_n[3w]*win_n[3w+1]*win_n[3w+2] entries). */
+int psdo_deposit_windows(const void *pos, int dtype, int stride, int N, double L, double M, int G,
+                         int K, const int64_t *win_lo, const int64_t *win_n, double *out, int mode) {
+    if (N < 2 || G < 1 || !(L > 0) || (stride != 3 && stride != 4) || K < 1 || K > 64) return 1;
+    target_t T[64];
+    size_t off = 0;
+    for (int w = 0; w < K; ++w) {
+        for (int x = 0; x < 3; ++x)
+            if (win_n[3 * w + x] < 1 || win_n[3 * w + x] > G) return 1;
+        target_t t = {G, out + off, 1, {win_lo[3 * w], win_lo[3 * w + 1], win_lo[3 * w + 2]},
+                      {win_n[3 * w], win_n[3 * w + 1], win_n[3 * w + 2]}};
+        T[w] = t;
+        off += (size_t)(win_n[3 * w] * win_n[3 * w + 1] * win_n[3 * w + 2]);
+    }
+    memset(out, 0, sizeof(double) * off);
+    particles_t p = {pos, dtype, stride, N, L};
+    const double m = M / (6.0 * (double)N * (double)N * (double)N);
+    const REAL scale = (REAL)G / (REAL)L;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j)
+            for (int k = 0; k < N; ++k) {
+                REAL P[8][3];
+                cell_corners(&p, i, j, k, P);
+                for (int t = 0; t < 6; ++t) {
+                    tet_t tet;
+                    make_tet(P, t, scale, &tet);
+                    for (int w = 0; w < K; ++w) deposit_tet(&tet, m, mode, &T[w], NULL, NULL, NULL);
+                }
+            }
+    return 0;
+}
+
+/* Where the method's hard places are (used to aim the windows of the full-size parity tests):
+ *   out[0..3]  = (i, j, k, t) of the tet with the largest cell range (ties: the first)
+ *   out[4..6]  = its lo cell;  out[7] = its number of cells
+ *   out[8..11] = (i, j, k, t) of the thinnest tet: smallest |det| / (product of the AABB edge
+ *                lengths in cells), among non-degenerate tets whose range has >= min_cells cells
+ *   out[12..14] = its lo cell; thin_out = that ratio                                          */
+int psdo_extreme_tets(const void *pos, int dtype, int stride, int N, double L, int G,
+                      int64_t min_cells, int64_t *out, double *thin_out) {
+    if (N < 2 || G < 1) return 1;
+    particles_t p = {pos, dtype, stride, N, L};
+    const REAL scale = (REAL)G / (REAL)L;
+    int64_t best_n = -1, bi[4] = {0, 0, 0, 0}, blo[3] = {0, 0, 0};
+    double best_thin = 1e300;
+    int64_t ti[4] = {0, 0, 0, 0}, tlo[3] = {0, 0, 0};
+    for (int i = 0; i < N; ++i) {
+        int64_t r_n = -1, r_i[4] = {0, 0, 0, 0}, r_lo[3] = {0, 0, 0};
+        double r_thin = 1e300;
+        int64_t s_i[4] = {0, 0, 0, 0}, s_lo[3] = {0, 0, 0};
+#pragma omp parallel
+        {
+            int64_t m_n = -1, m_i[4] = {0, 0, 0, 0}, m_lo[3] = {0, 0, 0};
+            double m_thin = 1e300;
+            int64_t q_i[4] = {0, 0, 0, 0}, q_lo[3] = {0, 0, 0};
+#pragma omp for schedule(static)
+            for (int j = 0; j < N; ++j)
+                for (int k = 0; k < N; ++k) {
+                    REAL P[8][3];
+                    cell_corners(&p, i, j, k, P);
+                    for (int t = 0; t < 6; ++t) {
+                        tet_t tet;
+                        make_tet(P, t, scale, &tet);
+                        int64_t n = 1;
+                        double box = 1.0;
+                        for (int x = 0; x < 3; ++x) {
+                            n *= tet.hi[x] - tet.lo[x] + 1;
+                            REAL mn = tet.g[0][x], mx = tet.g[0][x];
+                            for (int v = 1; v < 4; ++v) {
+                                if (tet.g[v][x] < mn) mn = tet.g[v][x];
+                                if (tet.g[v][x] > mx) mx = tet.g[v][x];
+                            }
+                            box *= (double)(mx - mn);
+                        }
+                        if (n > m_n) {
+                            m_n = n; m_i[0] = i; m_i[1] = j; m_i[2] = k; m_i[3] = t;
+                            for (int x = 0; x < 3; ++x) m_lo[x] = tet.lo[x];
+                        }
+                        double d = (double)(tet.det < 0 ? -tet.det : tet.det);
+                        if (n >= min_cells && d > 0 && box > 0 && d / box < m_thin) {
+                            m_thin = d / box; q_i[0] = i; q_i[1] = j; q_i[2] = k; q_i[3] = t;
+                            for (int x = 0; x < 3; ++x) q_lo[x] = tet.lo[x];
+                        }
+                    }
+                }
+#pragma omp critical
+            {
+                /* ties by (j,k,t) order: keep the smallest flat index */
+                int64_t key_m = (m_i[1] * N + m_i[2]) * 6 + m_i[3], key_r = (r_i[1] * N + r_i[2]) * 6 + r_i[3];
+                if (m_n > r_n || (m_n == r_n && m_n >= 0 && key_m < key_r)) {
+                    r_n = m_n;
+                    for (int x = 0; x < 4; ++x) r_i[x] = m_i[x];
+                    for (int x = 0; x < 3; ++x) r_lo[x] = m_lo[x];
+                }
+                if (m_thin < r_thin) {
+                    r_thin = m_thin;
+                    for (int x = 0; x < 4; ++x) s_i[x] = q_i[x];
+                    for (int x = 0; x < 3; ++x) s_lo[x] = q_lo[x];
+                }
+            }
+        }
+        if (r_n > best_n) {
+            best_n = r_n;
+            for (int x = 0; x < 4; ++x) bi[x] = r_i[x];
+            for (int x = 0; x < 3; ++x) blo[x] = r_lo[x];
+        }
+        if (r_thin < best_thin) {
+            best_thin = r_thin;
+            for (int x = 0; x < 4; ++x) ti[x] = s_i[x];
+            for (int x = 0; x < 3; ++x) tlo[x] = s_lo[x];
+        }
+    }
+    for (int x = 0; x < 4; ++x) { out[x] = bi[x]; out[8 + x] = ti[x]; }
+    for (int x = 0; x < 3; ++x) { out[4 + x] = blo[x]; out[12 + x] = tlo[x]; }
+    out[7] = best_n;
+    if (thin_out) *thin_out = best_thin;
+    return 0;
+}
+
 /* ---- single-tet entry points used by the pins -------------------------------- */
 
 /* vol(T n [lo, lo+h]^3) for an arbitrary tet given in any units (12 doubles, v-major). */

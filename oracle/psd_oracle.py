@@ -163,6 +163,73 @@ def census(pos, L: float, G: int, tile: int = TILE):
             "n_inverted": int(sc[4])}
 
 
+def census_classes(pos, L: float, G: int, tile: int = TILE, small_max: int = 8, win_lo=None, win_n=None):
+    """The census at full size (OpenMP over Lagrangian slabs), per tile split by the a3 size class
+    of the pair, optionally only for a window of tiles (wrapped tile coordinates)."""
+    p, dt, stride, N = _pos_args(pos)
+    nt = G // tile
+    wl = np.asarray(win_lo if win_lo is not None else (0, 0, 0), dtype=np.int64)
+    wn = np.asarray(win_n if win_n is not None else (nt, nt, nt), dtype=np.int64)
+    shape = tuple(int(x) for x in wn)
+    cs = np.zeros(shape, dtype=np.uint32)
+    cl = np.zeros(shape, dtype=np.uint32)
+    ht = np.zeros(64, dtype=np.uint64)
+    hp = np.zeros(64, dtype=np.uint64)
+    sc = np.zeros(8, dtype=np.int64)
+    lib = _lib()
+    u32p, u64p = C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
+    lib.psdo_census_classes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int,
+                                        C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_int64), u32p, u32p,
+                                        u64p, u64p, C.POINTER(C.c_int64)]
+    windowed = win_lo is not None
+    rc = lib.psdo_census_classes(p, dt, stride, N, L, G, tile, small_max,
+                                 _i64p(wl) if windowed else None, _i64p(wn) if windowed else None,
+                                 cs.ctypes.data_as(u32p), cl.ctypes.data_as(u32p),
+                                 ht.ctypes.data_as(u64p), hp.ctypes.data_as(u64p), _i64p(sc))
+    if rc:
+        raise ValueError(f"psdo_census_classes: rc={rc}")
+    return {"counts_small": cs, "counts_large": cl, "hist_tet": ht, "hist_pair": hp, "n_tets": int(sc[0]),
+            "n_pairs": int(sc[1]), "sum_cells": int(sc[2]), "max_cells": int(sc[3]), "n_inverted": int(sc[4])}
+
+
+def deposit_windows(pos, L, M, G, windows, mode: int = MODE_MASS):
+    """Several windows [(lo, n), ...] of the grid in one pass over the tets (see deposit_window)."""
+    p, dt, stride, N = _pos_args(pos)
+    K = len(windows)
+    lo = np.array([w[0] for w in windows], dtype=np.int64).reshape(K, 3)
+    n = np.array([w[1] for w in windows], dtype=np.int64).reshape(K, 3)
+    sizes = [int(np.prod(r)) for r in n]
+    out = np.empty(sum(sizes), dtype=np.float64)
+    lib = _lib()
+    lib.psdo_deposit_windows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                         C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64),
+                                         C.POINTER(C.c_double), C.c_int]
+    rc = lib.psdo_deposit_windows(p, dt, stride, N, L, M, G, K, _i64p(lo), _i64p(n), _dp(out), mode)
+    if rc:
+        raise ValueError("psdo_deposit_windows: invalid argument")
+    res, o = [], 0
+    for r, sz in zip(n, sizes):
+        res.append(out[o:o + sz].reshape(tuple(int(x) for x in r)))
+        o += sz
+    return res
+
+
+def extreme_tets(pos, L: float, G: int, min_cells: int = 8):
+    """The tet with the largest cell range and the thinnest one (smallest |det| / AABB volume):
+    where the full-size parity tests aim their windows."""
+    p, dt, stride, N = _pos_args(pos)
+    out = np.zeros(16, dtype=np.int64)
+    thin = C.c_double(0.0)
+    lib = _lib()
+    lib.psdo_extreme_tets.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_int64,
+                                      C.POINTER(C.c_int64), C.POINTER(C.c_double)]
+    rc = lib.psdo_extreme_tets(p, dt, stride, N, L, G, min_cells, _i64p(out), C.byref(thin))
+    if rc:
+        raise ValueError("psdo_extreme_tets: invalid argument")
+    return {"largest": {"tet": tuple(out[0:4].tolist()), "lo": out[4:7].copy(), "n_cells": int(out[7])},
+            "thinnest": {"tet": tuple(out[8:12].tolist()), "lo": out[12:15].copy(), "ratio": thin.value}}
+
+
 def tet_box_volume(verts, lo, h: float, kind: str = "double") -> float:
     """vol(T n [lo,lo+h]^3) by iterative plane splitting."""
     v = np.ascontiguousarray(verts, dtype=np.float64).reshape(12)

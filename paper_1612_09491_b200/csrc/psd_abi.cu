@@ -25,8 +25,13 @@ struct DevBuf {
         p = nullptr; cap = 0;
         size_t want = bytes + bytes / 8 + 256;  // a little slack so small growth does not realloc
         cudaError_t e = cudaMalloc(&p, want);
-        if (e != cudaSuccess) { e = cudaMalloc(&p, bytes); want = bytes; }
+        if (e != cudaSuccess) {
+            cudaGetLastError();  // the failed attempt must not stay behind as the runtime's last error
+            e = cudaMalloc(&p, bytes);
+            want = bytes;
+        }
         if (e == cudaSuccess) cap = want;
+        else { p = nullptr; cudaGetLastError(); }
         return e;
     }
     void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
@@ -374,6 +379,7 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
     if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
     if (!ctx->built) return fail(ctx, PSD_ERR_STATE, "psd_deposit_patches before psd_build_tets");
     if (!patches_host || n_patch < 1 || !mass_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "NULL argument or no patches");
+    if (n_patch > 0x7fffffffll / 64) return fail(ctx, PSD_ERR_INVALID_ARG, "too many patches (tile ids are 32-bit)");
     if (P < TILE || P % TILE || base_G < P || base_G % P)
         return fail(ctx, PSD_ERR_INVALID_ARG, "P must be a multiple of 8 and divide base_G");
     CK(cudaSetDevice(ctx->device));
@@ -406,6 +412,8 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
         long long np = ((long long)base_G << l) / P;
         total += np * np * np;
     }
+    if (total > (1ll << 28))
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_deposit_patches: more than 2^28 patch positions on the listed levels");
     std::vector<int> lookup;
     std::vector<int> fam;                       // per refined patch: its index, then its 8 children
     std::vector<long long> fam_level_begin;     // first family of each level (families sorted by level)
@@ -495,12 +503,17 @@ int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double fa
     if (((long long)base_G << max_level) > 2048 * 8) return fail(ctx, PSD_ERR_INVALID_ARG, "level grid too fine");
     CK(cudaSetDevice(ctx->device));
     const int nl = max_level + 1;
-    std::vector<long long> off(nl + 1, 0);
-    std::vector<int> np(nl);
+    long long off[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int np[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (int l = 0; l < nl; ++l) {
         np[l] = (base_G << l) / P;
         off[l + 1] = off[l] + (long long)np[l] * np[l] * np[l];
     }
+    // the rule runs on the host over every candidate position: keep that bounded (and the patch
+    // indices inside int)
+    if (off[nl] > (1ll << 28))
+        return fail(ctx, PSD_ERR_INVALID_ARG, "psd_refine_patches: more than 2^28 candidate patch positions");
+  try {
     // one extra word at the end: boxes the sub-block census could not place
     CK(ctx->refine_counts.ensure(sizeof(unsigned long long) * (size_t)(off[nl] + 1)));
     CK(cudaMemsetAsync(ctx->refine_counts.p, 0, sizeof(unsigned long long) * (size_t)(off[nl] + 1), ctx->stream));
@@ -583,6 +596,9 @@ int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, double fa
     *n_out = n;
     if (out_host && n > cap) return fail(ctx, PSD_ERR_INVALID_ARG, "patch list capacity too small");
     return PSD_OK;
+  } catch (const std::bad_alloc&) {
+    return fail(ctx, PSD_ERR_OOM, "psd_refine_patches: host allocation failed");
+  }
 }
 
 int psd_deposit_uniform_host(psd_ctx* ctx, const void* pos_host, int dtype, int stride_elems, int N, double L,

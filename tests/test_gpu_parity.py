@@ -443,11 +443,68 @@ def window_of(grid_dev, lo, edge, G):
     return grid_dev[ix[0]][:, ix[1]][:, :, ix[2]].cpu().numpy()
 
 
-@pytest.mark.parametrize("cfg_index,n_win,edge", [(1, 6, 12), (2, 3, 10)])
-def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_win, edge):
+def aimed_windows(oracle, pos, G, edge, n_random, seed):
+    """Where the full-size tests look: across the periodic seam, around the densest region of the
+    particle distribution (a coarse histogram of the input positions), around the tet with the
+    largest cell range and around the thinnest tet (both found by the oracle), plus seeded
+    random windows.  Nothing here comes from the CUDA path."""
+    wins = {"seam": (G - 3, G - 5, 0)}
+    H = min(G, 256)
+    idx = np.floor(pos[..., :3].reshape(-1, 3).astype(np.float64) * H).astype(np.int64) % H
+    flat = (idx[:, 0] * H + idx[:, 1]) * H + idx[:, 2]
+    del idx
+    dense = int(np.bincount(flat, minlength=H ** 3).argmax())
+    del flat
+    d = np.array([dense // (H * H), (dense // H) % H, dense % H]) * (G // H) + (G // H) // 2
+    wins["densest"] = tuple(int(x) for x in (d - edge // 2) % G)
+    e = oracle.extreme_tets(pos, 1.0, G, min_cells=8)
+    wins["largest_tet"] = tuple(int(x) for x in (e["largest"]["lo"] - 2) % G)
+    wins["thinnest_tet"] = tuple(int(x) for x in (e["thinnest"]["lo"] - 2) % G)
+    rnd, _ = sample_windows(G, n_random, edge, seed)
+    for i, lo in enumerate(rnd):
+        wins[f"random{i}"] = tuple(int(x) for x in lo)
+    return wins, e
+
+
+def check_windows(oracle, pos, grid, G, wins, edge, mx):
+    names = list(wins)
+    oras = oracle.deposit_windows(pos, 1.0, 1.0, G, [(wins[k], (edge,) * 3) for k in names])
+    for k, ora in zip(names, oras):
+        err = np.abs(window_of(grid, wins[k], edge, G) - ora)
+        assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (k, wins[k], float(err.max()))
+        assert ora.max() > 0
+
+
+def check_census(oracle, ctx, pos, G, win_tiles=None):
+    """a2/a3 bit-exact: pairs per (tile, size class) of the last binned deposit against the oracle,
+    on every tile, or on windows of tiles; histograms and scalars when every tile is compared."""
+    s = ctx.psd_get_stats()
+    nt = G // 8
+    got = ctx.psd_get_tile_class_counts().reshape(nt, nt, nt, 2)
+    if win_tiles is None:
+        c = oracle.census_classes(pos, 1.0, G)
+        assert np.array_equal(got[..., 0], c["counts_small"]) and np.array_equal(got[..., 1], c["counts_large"])
+        assert np.array_equal(np.array(s.hist_tet, dtype=np.uint64), c["hist_tet"])
+        assert np.array_equal(np.array(s.hist_pair, dtype=np.uint64), c["hist_pair"])
+        assert (s.n_pairs, s.sum_cells, s.max_cells, s.n_inverted) == \
+            (c["n_pairs"], c["sum_cells"], c["max_cells"], c["n_inverted"])
+        return
+    for lo, n in win_tiles:
+        c = oracle.census_classes(pos, 1.0, G, win_lo=lo, win_n=n)
+        ix = np.ix_(*[(np.arange(n[a]) + lo[a]) % nt for a in range(3)])
+        assert np.array_equal(got[..., 0][ix], c["counts_small"]), lo
+        assert np.array_equal(got[..., 1][ix], c["counts_large"]), lo
+        assert c["n_pairs"] > 0
+        assert np.array_equal(np.array(s.hist_tet, dtype=np.uint64), c["hist_tet"])
+        assert (s.sum_cells, s.max_cells, s.n_inverted) == (c["sum_cells"], c["max_cells"], c["n_inverted"])
+
+
+@pytest.mark.parametrize("cfg_index,n_random,edge", [(1, 4, 12), (2, 2, 12)])
+def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_random, edge):
     """BASELINE.json configs[1], [2] at full size in the launch configuration bench.py times:
-    total mass, signed-volume cover of every cell, and oracle parity on sampled windows
-    (windows may wrap around the box)."""
+    total mass, signed-volume cover of every cell, pairs per (tile, size class) and census
+    histograms bit-exact on every tile, and oracle parity on windows aimed at the method's hard
+    places (windows may wrap around the box)."""
     import torch
     cfg = psd_inputs.CONFIGS[cfg_index]
     G = cfg["G"]
@@ -458,13 +515,10 @@ def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_win, edg
     assert_mass(grid.sum())
     assert float(grid.min()) > 0.0
     mx = float(grid.max())
-    wins, _ = sample_windows(G, n_win, edge, 1000 + cfg_index)
-    wins[0] = (G - 3, G - 5, 0)  # one window across the periodic seam
-    for lo in wins:
-        ora = oracle.deposit_window(pos, 1.0, 1.0, G, lo, (edge,) * 3)
-        got = window_of(grid, lo, edge, G)
-        err = np.abs(got - ora)
-        assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (lo, float(err.max()))
+    check_census(oracle, ctx, pos, G)
+    wins, ext = aimed_windows(oracle, pos, G, edge, n_random, 1000 + cfg_index)
+    assert ext["largest"]["n_cells"] == ctx.psd_get_stats().max_cells
+    check_windows(oracle, pos, grid, G, wins, edge, mx)
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
     ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
@@ -497,12 +551,16 @@ def test_cfg3_full_size_patches(psd, ctx, oracle):
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
     assert_mass(mass[torch.from_numpy(levels == 0).cuda()].sum())
-    # sampled patches, two per level (seeded), against the oracle
+    # sampled patches against the oracle: per level the hottest one (largest census count) and
+    # four seeded ones
     pick = []
     for l in range(max_level + 1):
         idx = np.nonzero(levels == l)[0]
-        u = psd_inputs.splitmix64(3000 + l, 0, 2) % np.uint64(len(idx))
+        cnt_l = np.array([int(ocounts[l][tuple(patches[i, 1:])]) for i in idx])
+        pick.append(int(idx[int(cnt_l.argmax())]))
+        u = psd_inputs.splitmix64(3000 + l, 0, 4) % np.uint64(len(idx))
         pick += [int(idx[int(x)]) for x in u]
+    pick = sorted(set(pick))
     ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches[pick])
     got = mass[torch.tensor(pick, device="cuda")].cpu().numpy()
     mx = float(mass.max())
@@ -542,11 +600,15 @@ def test_cfg4_full_size_uniform(psd, ctx, oracle):
     assert abs(total - 1.0) <= 1e-10, total
     assert float(grid.min()) > 0.0
     mx = float(grid.max())
-    edge = 8
-    for lo in [(G - 3, 5, G - 6), (417, 230, 771)]:
-        ora = oracle.deposit_window(pos, 1.0, 1.0, G, lo, (edge,) * 3)
-        err = np.abs(window_of(grid, lo, edge, G) - ora)
-        assert (err <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (lo, float(err.max()))
+    edge = 12
+    wins, ext = aimed_windows(oracle, pos, G, edge, 3, 1004)
+    assert ext["largest"]["n_cells"] == s.max_cells
+    check_windows(oracle, pos, grid, G, wins, edge, mx)
+    # pairs per (tile, size class) bit-exact on four regions of 8^3 tiles (64^3 cells) at those places
+    nt = G // 8
+    regions = [(tuple(int((c // 8 - 3) % nt) for c in wins[k]), (8, 8, 8))
+               for k in ("seam", "densest", "largest_tet", "thinnest_tet")]
+    check_census(oracle, ctx, pos, G, regions)
     ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
     ctx.psd_deposit_uniform(G, grid)
     assert float((grid - 1.0).abs().max()) < 1e-9
@@ -568,6 +630,24 @@ def test_paper_weak_scaling_workload_jittered_lattice(psd, ctx, oracle, kernel):
     assert_parity(g.cpu().numpy(), ora, what="jittered lattice")
     s = ctx.psd_get_stats()
     assert s.n_inverted == st["n_inverted"] > 0 and s.sum_cells == st["n_candidates"]
+
+
+def test_paper_weak_scaling_workload_at_its_quoted_size(psd, ctx, oracle):
+    """PAPER.md:175 at the size the paper quotes: 512^3 jittered particles onto 256^3 cells, the
+    launch configuration `bench.py --config 5` times.  Mass, positivity, aimed + random windows."""
+    import torch
+    cfg = psd_inputs.CONFIGS[5]
+    G = cfg["G"]
+    pos = psd_inputs.config_positions(5)
+    ctx.psd_build_tets(to_dev(pos))
+    grid = torch.empty((G, G, G), dtype=torch.float64, device="cuda")
+    ctx.psd_deposit_uniform(G, grid)
+    s = ctx.psd_get_stats()
+    assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    assert_mass(grid.sum())
+    assert float(grid.min()) > 0.0
+    wins, _ = aimed_windows(oracle, pos, G, 12, 2, 1005)
+    check_windows(oracle, pos, grid, G, wins, 12, float(grid.max()))
 
 
 @pytest.mark.parametrize("N", [2, 3])

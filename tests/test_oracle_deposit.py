@@ -396,3 +396,80 @@ def test_refine_rule_bottom_up_hand_built():
     want |= {(1, 2 + a, b, c) for a in range(2) for b in range(2) for c in range(2)}      # children of (0,1,0,0)
     want |= {(2, 4 + a, b, 2 + c) for a in range(2) for b in range(2) for c in range(2)}  # children of (1,2,0,1)
     assert got == want
+
+
+# ------------------------------------------------------------------ helpers of the full-size parity tests
+def test_census_classes_equals_the_plain_census(oracle):
+    """psdo_census_classes (parallel, split by size class, optional tile window) against the plain
+    serial psdo_census and a python recount of the class split, on a field that wraps around."""
+    N, G = 8, 32
+    pos = crossing_field(N, 2.0)
+    c = oracle.census(pos, 1.0, G)
+    f = oracle.census_classes(pos, 1.0, G)
+    nt = G // 8
+    assert np.array_equal((f["counts_small"] + f["counts_large"]).ravel(), c["tile_counts"])
+    for k in ("hist_tet", "hist_pair"):
+        assert np.array_equal(f[k], c[k])
+    for k in ("n_tets", "n_pairs", "sum_cells", "max_cells", "n_inverted"):
+        assert f[k] == c[k]
+    # the class split: small = buckets 0..3 of hist_pair (<= 8 cells), per tile by a python recount
+    assert int(f["counts_small"].sum()) == int(c["hist_pair"][:4].sum())
+    small = np.zeros((nt, nt, nt), dtype=np.int64)
+    for i in range(N):
+        for j in range(N):
+            for k in range(N):
+                for t in range(6):
+                    _, _, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+                    per_axis = []
+                    for a in range(3):
+                        d = {}
+                        for cc in range(int(lo[a]), int(hi[a]) + 1):
+                            d[(cc % G) // 8] = d.get((cc % G) // 8, 0) + 1
+                        per_axis.append(d)
+                    for tx, nx in per_axis[0].items():
+                        for ty, ny in per_axis[1].items():
+                            for tz, nz in per_axis[2].items():
+                                small[tx, ty, tz] += nx * ny * nz <= 8
+    assert np.array_equal(small, f["counts_small"].astype(np.int64))
+    # a window of tiles that wraps around the box
+    w = oracle.census_classes(pos, 1.0, G, win_lo=(3, 0, 2), win_n=(2, 4, 1))
+    idx = np.ix_([3, 0], range(4), [2])
+    assert np.array_equal(w["counts_small"], f["counts_small"][idx])
+    assert np.array_equal(w["counts_large"], f["counts_large"][idx])
+    assert w["n_pairs"] == int(w["counts_small"].sum() + w["counts_large"].sum()) == int(w["hist_pair"].sum())
+    assert np.array_equal(w["hist_tet"], f["hist_tet"])
+    # another threshold
+    g = oracle.census_classes(pos, 1.0, G, small_max=64)
+    assert int(g["counts_small"].sum()) == int(c["hist_pair"][:7].sum())
+
+
+def test_deposit_windows_equals_single_windows(oracle):
+    pos = crossing_field(6, 1.5)
+    G = 12
+    wins = [((10, 3, 0), (4, 5, 12)), ((0, 0, 0), (3, 3, 3)), ((11, 11, 11), (2, 2, 2))]
+    many = oracle.deposit_windows(pos, 1.0, 1.0, G, wins)
+    for (lo, n), got in zip(wins, many):
+        assert np.allclose(got, oracle.deposit_window(pos, 1.0, 1.0, G, lo, n), rtol=1e-12, atol=1e-18)
+
+
+def test_extreme_tets_against_a_python_scan(oracle):
+    N, G = 8, 32
+    pos = crossing_field(N, 2.5)
+    e = oracle.extreme_tets(pos, 1.0, G, min_cells=8)
+    best_n, best_thin, thin_tet = -1, np.inf, None
+    for i in range(N):
+        for j in range(N):
+            for k in range(N):
+                for t in range(6):
+                    verts, det, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+                    n = int(np.prod(hi - lo + 1))
+                    best_n = max(best_n, n)
+                    g = verts * G
+                    box = float(np.prod(g.max(0) - g.min(0)))
+                    if n >= 8 and det != 0 and abs(det) / box < best_thin:
+                        best_thin, thin_tet = abs(det) / box, (i, j, k, t)
+    assert e["largest"]["n_cells"] == best_n
+    i, j, k, t = e["largest"]["tet"]
+    _, _, lo, hi = oracle.build_tet(pos, 1.0, G, i, j, k, t)
+    assert int(np.prod(hi - lo + 1)) == best_n and np.array_equal(lo, e["largest"]["lo"])
+    assert e["thinnest"]["tet"] == thin_tet and np.isclose(e["thinnest"]["ratio"], best_thin, rtol=1e-12)
