@@ -18,8 +18,11 @@
  *    counters), grown on demand and reused between calls.
  *  - Every function returns a psd_status (0 = PSD_OK); nothing throws or exits.
  *    psd_last_error() gives a human-readable string for the last failure on that context.
- *  - Work is enqueued on the context's CUDA stream and is asynchronous unless stated;
- *    psd_sync / psd_get_stats / psd_refine_patches / *_host calls synchronise.
+ *  - Work is enqueued on the context's CUDA stream.  psd_sync / psd_get_stats /
+ *    psd_refine_patches / psd_build_tets / *_host calls synchronise with it.  The deposits return
+ *    with the clip-and-deposit kernel still running, but on the binned path they block the
+ *    host ONCE in between, after the census and the scan, to read the two list sizes that size
+ *    the scratch and the launch (so they cannot be captured into a CUDA graph).
  *  - One context is used from one host thread at a time.
  *  - There is no CPU fallback: without a CUDA device psd_create fails.
  */
@@ -46,7 +49,8 @@ typedef enum {
     PSD_ERR_STATE = 2,       /* deposit or refine before psd_build_tets             */
     PSD_ERR_OOM = 3,         /* scratch allocation failed                           */
     PSD_ERR_CUDA = 4,        /* a CUDA call or kernel failed (see psd_last_error)   */
-    PSD_ERR_UNWRAP = 5       /* reserved: minimum-image unwrap not valid            */
+    PSD_ERR_UNWRAP = 5       /* psd_refine_patches with the sub-block census: a sub-block's
+                                bounding box is too long for the minimum-image unwrap   */
 } psd_status;
 
 enum { PSD_F32 = 0, PSD_F64 = 1 };
@@ -106,7 +110,9 @@ typedef struct {
     int64_t max_cells;    /* largest AABB                                                */
     int64_t n_inverted;   /* tets with negative determinant                */
     int64_t n_degenerate; /* tets with determinant exactly 0                             */
-    int64_t n_unwrap_suspect; /* unwrapped Lagrangian cell edges longer than L/4         */
+    int64_t n_unwrap_suspect; /* Lagrangian cells with an unwrapped edge longer than L/4: the
+                             minimum image is only valid below L/2 (Q4).  Advisory:
+                             counted on both paths, never an error                          */
     int64_t n_nonfinite;  /* NaN/Inf position components seen by psd_build_tets          */
     uint64_t hist_tet[64];  /* tets by b = bit_width(n_cells-1)                          */
     uint64_t hist_pair[64]; /* pairs by b of the tet's cells inside that tile            */
@@ -150,7 +156,7 @@ PSD_API int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int str
  *   G          cells per side (>= 1); cell (ix,iy,iz) spans [ix,ix+1)*L/G ...
  *   grid_dev   G^3 doubles, index (ix*G+iy)*G+iz, MASS per cell (not density).
  *   accumulate 0: the library zeroes the grid first; 1: adds to what is there.
- * Asynchronous. */
+ * Returns with the deposit kernel enqueued (one host round trip for the list sizes, see above). */
 PSD_API int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate);
 
 /* PAPER.md:66 (refinement by tet count), :72 (leaf patches).  Census-driven construction of
@@ -171,7 +177,8 @@ PSD_API int psd_refine_patches(psd_ctx* ctx, int base_G, int P, int max_level, d
  *   patches_host  n_patch patches (host; copied), distinct
  *   P             cells per patch side, multiple of 8;  base_G % P == 0
  *   mass_dev      n_patch * P^3 doubles, patch-major then (x*P+y)*P+z
- * Asynchronous (the patch list is copied before return). */
+ * Returns with the deposit (and restriction) kernels enqueued; the patch list is copied before
+ * return; one host round trip for the list sizes, see above. */
 PSD_API int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_patch, int P,
                         int base_G, double* mass_dev, int accumulate);
 

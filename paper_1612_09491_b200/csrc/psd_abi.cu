@@ -55,7 +55,7 @@ struct psd_ctx {
     psd_stats last{};
     bool stats_pending = false;
     bool binned_last = false;
-    std::string err;
+    char err[384] = "";
     int64_t launches = 0;
     cudaEvent_t ev[6] = {};
     // psd_deposit_uniform_host: the grid goes back to the host slab by slab while later slabs are
@@ -69,13 +69,17 @@ struct psd_ctx {
 
 namespace {
 
-int fail(psd_ctx* c, int code, const std::string& msg) {
-    if (c) c->err = msg;
+int fail(psd_ctx* c, int code, const char* msg) {  // nothing here may throw across the C ABI
+    if (c) {
+        std::snprintf(c->err, sizeof(c->err), "%s", msg);
+    }
     return code;
 }
 int cuda_fail(psd_ctx* c, cudaError_t e, const char* what) {
-    return fail(c, e == cudaErrorMemoryAllocation ? PSD_ERR_OOM : PSD_ERR_CUDA,
-                std::string(what) + ": " + cudaGetErrorString(e));
+    char buf[320];
+    std::snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
+    if (e == cudaErrorMemoryAllocation) cudaGetLastError();  // reported; do not leave it for the next check
+    return fail(c, e == cudaErrorMemoryAllocation ? PSD_ERR_OOM : PSD_ERR_CUDA, buf);
 }
 #define CK(call)                                                    \
     do {                                                            \
@@ -379,7 +383,11 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
     if (!valid_ctx(ctx)) return PSD_ERR_INVALID_ARG;
     if (!ctx->built) return fail(ctx, PSD_ERR_STATE, "psd_deposit_patches before psd_build_tets");
     if (!patches_host || n_patch < 1 || !mass_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "NULL argument or no patches");
-    if (n_patch > 0x7fffffffll / 64) return fail(ctx, PSD_ERR_INVALID_ARG, "too many patches (tile ids are 32-bit)");
+    {
+        const long long tp = P / TILE;
+        if ((long double)n_patch * tp * tp * tp * N_CLASSES > 2147483647.0L)
+            return fail(ctx, PSD_ERR_INVALID_ARG, "too many patches: (tile, size class) bins are indexed with 32 bits");
+    }
     if (P < TILE || P % TILE || base_G < P || base_G % P)
         return fail(ctx, PSD_ERR_INVALID_ARG, "P must be a multiple of 8 and divide base_G");
     CK(cudaSetDevice(ctx->device));
@@ -705,13 +713,17 @@ int psd_get_tile_counts(psd_ctx* ctx, uint32_t* out_host, int64_t cap) {
     if (!valid_ctx(ctx) || !out_host) return PSD_ERR_INVALID_ARG;
     if (!ctx->binned_last || ctx->last.n_tiles <= 0) return fail(ctx, PSD_ERR_STATE, "no binned deposit to report");
     if (cap < ctx->last.n_tiles) return fail(ctx, PSD_ERR_INVALID_ARG, "tile count buffer too small");
-    std::vector<uint32_t> bins((size_t)ctx->last.n_tiles * N_CLASSES);
-    int rc = psd_get_tile_class_counts(ctx, bins.data(), (int64_t)bins.size());
-    if (rc) return rc;
-    for (int64_t t = 0; t < ctx->last.n_tiles; ++t) {
-        uint32_t c = 0;
-        for (int k = 0; k < N_CLASSES; ++k) c += bins[(size_t)t * N_CLASSES + k];
-        out_host[t] = c;
+    try {
+        std::vector<uint32_t> bins((size_t)ctx->last.n_tiles * N_CLASSES);
+        int rc = psd_get_tile_class_counts(ctx, bins.data(), (int64_t)bins.size());
+        if (rc) return rc;
+        for (int64_t t = 0; t < ctx->last.n_tiles; ++t) {
+            uint32_t c = 0;
+            for (int k = 0; k < N_CLASSES; ++k) c += bins[(size_t)t * N_CLASSES + k];
+            out_host[t] = c;
+        }
+    } catch (const std::bad_alloc&) {
+        return fail(ctx, PSD_ERR_OOM, "psd_get_tile_counts: host allocation failed");
     }
     return PSD_OK;
 }
@@ -756,7 +768,7 @@ int psd_sync(psd_ctx* ctx) {
     return PSD_OK;
 }
 
-const char* psd_last_error(const psd_ctx* ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+const char* psd_last_error(const psd_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
 
 int64_t psd_launch_count(const psd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

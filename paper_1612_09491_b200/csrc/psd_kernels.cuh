@@ -954,7 +954,7 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
     int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     unsigned long long nc = 0;
-    unsigned int inv = 0, deg = 0;
+    unsigned int inv = 0, deg = 0, suspect = 0;
     if (id < ntet) {
         double P[4][3];
         load_tet_vertices(p, id / 6, (int)(id % 6), P);
@@ -964,6 +964,19 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
         atomicAdd(&sh_hist[bit_width_u64(nc - 1)], 1u);
         double det = tet_det_sign(t.g);
         inv = det < 0.0; deg = det == 0.0;
+        if (id % 6 == 0) {  // once per Lagrangian cell: its three edges from corner 0 (as in k_census)
+            const int64_t cell = id / 6;
+            const int N = p.N;
+            const int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((int64_t)N * N));
+            double c0[3], c[3];
+            load_pos(p, corner_index(i, j, k, 0, N), c0);
+#pragma unroll
+            for (int b = 1; b <= 4; b <<= 1) {
+                load_pos(p, corner_index(i, j, k, b, N), c);
+#pragma unroll
+                for (int x = 0; x < 3; ++x) suspect |= fabs(unwrap1(c[x], c0[x], p.L) - c0[x]) > 0.25 * p.L;
+            }
+        }
     }
     // warp partials (64-bit sum and max by halves), then one shared atomic per warp
     unsigned long long sum = nc, mx = nc;
@@ -974,11 +987,13 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
     }
     inv = __reduce_add_sync(0xffffffffu, inv);
     deg = __reduce_add_sync(0xffffffffu, deg);
+    suspect = __reduce_add_sync(0xffffffffu, suspect);
     if ((threadIdx.x & 31) == 0) {
         atomicAdd(&sh_stat[ST_SUM_CELLS], sum);
         atomicMax(&sh_stat[ST_MAX_CELLS], mx);
         if (inv) atomicAdd(&sh_stat[ST_INVERTED], (unsigned long long)inv);
         if (deg) atomicAdd(&sh_stat[ST_DEGENERATE], (unsigned long long)deg);
+        if (suspect) atomicAdd(&sh_stat[ST_UNWRAP], (unsigned long long)suspect);
     }
     __syncthreads();
     if (threadIdx.x < 64 && sh_hist[threadIdx.x]) atomicAdd(&hist[threadIdx.x], (unsigned long long)sh_hist[threadIdx.x]);
@@ -986,6 +1001,7 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
     if (threadIdx.x == ST_MAX_CELLS) atomicMax(&stats[ST_MAX_CELLS], sh_stat[ST_MAX_CELLS]);
     if (threadIdx.x == ST_INVERTED && sh_stat[ST_INVERTED]) atomicAdd(&stats[ST_INVERTED], sh_stat[ST_INVERTED]);
     if (threadIdx.x == ST_DEGENERATE && sh_stat[ST_DEGENERATE]) atomicAdd(&stats[ST_DEGENERATE], sh_stat[ST_DEGENERATE]);
+    if (threadIdx.x == ST_UNWRAP && sh_stat[ST_UNWRAP]) atomicAdd(&stats[ST_UNWRAP], sh_stat[ST_UNWRAP]);
 }
 
 // ---------------------------------------------------------------- a7 refinement census

@@ -320,6 +320,19 @@ def test_patch_restriction_fills_refined_parents_from_their_children(psd, ctx, o
     assert_parity(0.5 * m, oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches), what="accumulated")
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_unwrap_suspects_are_counted_on_both_paths(psd, ctx, kernel):
+    """Q4: the minimum image is valid while every Lagrangian cell edge is shorter than L/2; cells with
+    an edge longer than L/4 are counted (advisory).  N = 3: every edge is L/3; N = 8: L/8."""
+    ctx.psd_set_option(psd.OPT_KERNEL, kernel)
+    ctx.psd_build_tets(to_dev(psd_inputs.lattice(3, shift=(0.01, 0.02, 0.03))))
+    ctx.psd_deposit_uniform(8)
+    assert ctx.psd_get_stats().n_unwrap_suspect == 27
+    ctx.psd_build_tets(to_dev(psd_inputs.lattice(8, shift=(0.01, 0.02, 0.03))))
+    ctx.psd_deposit_uniform(8)
+    assert ctx.psd_get_stats().n_unwrap_suspect == 0
+
+
 def test_error_codes(psd, ctx):
     import torch
     with pytest.raises(psd.PsdError) as e:
