@@ -443,16 +443,16 @@ __device__ __forceinline__ double tile_value(const double* cell, double inv_scal
 }
 
 #ifndef DEP_MIN_CTAS
-#define DEP_MIN_CTAS 3
+#define DEP_MIN_CTAS 4
 #endif
 #ifndef DEP_WARPS_N
-#define DEP_WARPS_N 6
+#define DEP_WARPS_N 4
 #endif
 constexpr int DEP_WARPS = DEP_WARPS_N;
 constexpr int DEP_THREADS = DEP_WARPS * 32;
 // per-warp scratch in doubles: tet slots [13][32] (12 tile-local coordinates + weight), polygon
-// [3*LB_SLOTS][32], face rectangles [32] (u64), slot words [32] (u32)
-constexpr int WARP_SCRATCH = (13 + 3 * LB_SLOTS) * 32 + 32 + 16;
+// [3*LB_SLOTS][32], per-face row ranges [4][32] (u64), slot words [32] (u32)
+constexpr int WARP_SCRATCH = (13 + 3 * LB_SLOTS) * 32 + 4 * 32 + 16;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
 
 // The general convex clip (clip_wall) of one face job, for the jobs the straight-line clip
@@ -501,8 +501,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
     double* wpoly = wtet + 13 * 32;                                                    // [3 * LB_SLOTS][32]
-    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [32]
-    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 32);                 // [32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [4][32]
+    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 4 * 32);             // [32]
     PolyBuf<32> poly{wpoly + lane};
     // slots 6..9 of the lane's polygon buffer hold the corners of the column's unit square: their
     // (v, w) never change (the general clip may overwrite slot 6: restored before the next job)
@@ -582,7 +582,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     ax = (e0 >= e1 && e0 >= e2) ? 0 : (e1 >= e2 ? 1 : 2);
                 }
                 const int av = (ax + 1) % 3, aw = (ax + 2) % 3;
-                unsigned long long rect = 0ull;
+                bool rect_written = false;
                 if (det == 0.0) {  // degenerate: whole mass to the centroid cell (Q6)
                     if (A.weight_mode == 0) {
                         int c[3];
@@ -605,6 +605,11 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     // runtime axis (the lane's own stores above); the faces' rectangles are then
                     // integer min / max (floor and ceil are monotone)
                     int fv[4], cvv[4], fw[4], cww[4], cuu[4];
+                    // the same with a margin (a point within ROW_EPS of a lattice line counts for both
+                    // sides): rows / columns a vertex belongs to, for the per-row column ranges
+                    int rlo[4], rhi[4], klo[4], khi[4];
+                    double pvv[4], pww[4];
+                    constexpr double ROW_EPS = 1e-9;
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
                         const double pu = wtet[(3 * v + ax) * 32 + lane], pv = wtet[(3 * v + av) * 32 + lane];
@@ -612,31 +617,79 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         fv[v] = __double2int_rd(pv); cvv[v] = __double2int_ru(pv);
                         fw[v] = __double2int_rd(pw); cww[v] = __double2int_ru(pw);
                         cuu[v] = __double2int_ru(pu);
+                        rlo[v] = __double2int_rd(pv - ROW_EPS); rhi[v] = __double2int_rd(pv + ROW_EPS);
+                        klo[v] = __double2int_rd(pw - ROW_EPS); khi[v] = __double2int_rd(pw + ROW_EPS);
+                        pvv[v] = pv; pww[v] = pw;
                     }
                     const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
                     const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
                     const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
                     const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
                     const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
+                    // dw/dv of the 6 edges (i < j), index i + j - (i == 0 ? 1 : 0): 01 02 03 12 13 23
+                    double slope[6];
+#pragma unroll
+                    for (int i = 0; i < 3; ++i)
+#pragma unroll
+                        for (int j = i + 1; j < 4; ++j) {
+                            const double dvv = pvv[j] - pvv[i];
+                            slope[i + j - (i == 0 ? 1 : 0)] = (pww[j] - pww[i]) * fast_rcp(dvv == 0.0 ? 1.0 : dvv);
+                        }
+                    // columns met by the face's three edges on the lattice line v = L (with the margin)
+                    auto line_cols = [&](const int a, const int b, const int d, const int L, int& clo, int& chi) {
+                        clo = 99; chi = -99;
+                        const int e0[3] = {a, b, a}, e1[3] = {b, d, d};   // edges with i < j: (a,b) (b,d) (a,d)
+#pragma unroll
+                        for (int e = 0; e < 3; ++e) {
+                            const int i = e0[e], j = e1[e];
+                            const double di = pvv[i] - (double)L, dj = pvv[j] - (double)L;
+                            if (di * dj < 0.0) {
+                                const double w = fma(-di, slope[i + j - (i == 0 ? 1 : 0)], pww[i]);
+                                clo = min(clo, __double2int_rd(w - ROW_EPS));
+                                chi = max(chi, __double2int_rd(w + ROW_EPS));
+                            }
+                        }
+                    };
 #pragma unroll
                     for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
-                        const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;
+                        const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;   // a < b < d
                         // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
                         const int v0 = max(min(min(fv[a], fv[b]), fv[d]), lov);
                         const int v1 = min(max(max(cvv[a], cvv[b]), cvv[d]) - 1, hiv);
                         const int w0 = max(min(min(fw[a], fw[b]), fw[d]), low);
                         const int w1 = min(max(max(cww[a], cww[b]), cww[d]) - 1, hiw);
                         int c = 0;
+                        unsigned long long rows = 0ull;
                         if (v1 >= v0 && w1 >= w0 && max(max(cuu[a], cuu[b]), cuu[d]) > lou) {
-                            c = (v1 - v0 + 1) * (w1 - w0 + 1);
-                            rect |= (unsigned long long)(v0 | (v1 - v0) << 3 | w0 << 6 | (w1 - w0) << 9) << (16 * f);
+                            // per row of the rectangle, the columns the triangle really meets: the
+                            // w-extremes of (triangle n row strip) are at vertices inside the strip or
+                            // where an edge crosses one of the strip's two lines -- no empty jobs
+                            rows = (unsigned long long)v0;
+                            int llo, lhi;
+                            line_cols(a, b, d, v0, llo, lhi);
+#pragma unroll 1
+                            for (int r = v0; r <= v1; ++r) {
+                                int ulo, uhi;
+                                line_cols(a, b, d, r + 1, ulo, uhi);
+                                int rl = min(llo, ulo), rh = max(lhi, uhi);
+                                if (rlo[a] <= r && r <= rhi[a]) { rl = min(rl, klo[a]); rh = max(rh, khi[a]); }
+                                if (rlo[b] <= r && r <= rhi[b]) { rl = min(rl, klo[b]); rh = max(rh, khi[b]); }
+                                if (rlo[d] <= r && r <= rhi[d]) { rl = min(rl, klo[d]); rh = max(rh, khi[d]); }
+                                const int c0 = max(rl, w0), c1 = min(rh, w1);
+                                const int n = max(c1 - c0 + 1, 0);
+                                rows |= (unsigned long long)(n ? (c0 | n << 3) : 0) << (3 + 7 * (r - v0));
+                                c += n;
+                                llo = ulo; lhi = uhi;
+                            }
                         }
                         cnts |= (unsigned int)c << (8 * f);
+                        wrect[f * 32 + lane] = rows;
                     }
+                    rect_written = true;
                 }
                 const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
                 const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
-                wrect[lane] = rect;
+                if (!rect_written) { wrect[lane] = 0ull; wrect[32 + lane] = 0ull; wrect[64 + lane] = 0ull; wrect[96 + lane] = 0ull; }
                 wword[lane] = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
             // ---- stages B + C for 32 jobs (a lambda with a single call site: its code is large).
@@ -783,15 +836,19 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 int cv = 0, cw = 0;
                 const bool act = job < total;
                 if (act) {
-                    // decode (slot, column)
-                    const int local = job - spre;
-                    const unsigned int r16 = (unsigned int)(wrect[slot] >> (16 * f)) & 0xffffu;
-                    const int nw = ((r16 >> 9) & 7) + 1;
-                    // local / nw for local < 64, nw <= 8 without an integer division:
-                    // (local * ceil(256 / nw)) >> 8 is exact there; the table holds ceil(256/nw) - 1
-                    const int inv = (int)((0x1f242a333f557fffull >> (8 * (nw - 1))) & 255ull) + 1;
-                    const int lq = (local * inv) >> 8;
-                    cv = (r16 & 7) + lq; cw = ((r16 >> 6) & 7) + (local - lq * nw);
+                    // decode (slot, row, column): bits 0..2 of the face's word = first row, then 7 bits
+                    // per row = first column (3) and number of columns (4)
+                    int local = job - spre;
+                    unsigned long long rw = wrect[f * 32 + slot];
+                    cv = (int)(rw & 7ull);
+                    rw >>= 3;
+#pragma unroll
+                    for (int r = 0; r < TILE; ++r) {
+                        const int n = (int)(rw >> 3) & 15;
+                        if (local < n) break;
+                        local -= n; ++cv; rw >>= 7;
+                    }
+                    cw = ((int)rw & 7) + local;
                 }
                 run_jobs(act, slot, f, cv, cw);
             }
