@@ -339,6 +339,10 @@ int psd_build_tets(psd_ctx* ctx, const void* pos_dev, int dtype, int stride_elem
     ctx->part.stride = stride_elems;
     ctx->part.N = N;
     ctx->part.L = L;
+    {
+        int e = 0;
+        ctx->part.inv_L = std::frexp(L, &e) == 0.5 ? 1.0 / L : 0.0;  // exact reciprocal of a power of two
+    }
     ctx->total_mass = total_mass;
     int rc = reset_stats(ctx);
     if (rc) return rc;

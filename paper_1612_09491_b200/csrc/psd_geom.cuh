@@ -42,6 +42,7 @@ struct Particles {
     int stride;  // 3 or 4
     int N;
     double L;
+    double inv_L;  // 1 / L when L is a power of two (then x * inv_L == x / L exactly), else 0
 };
 
 __device__ __forceinline__ void load_pos(const Particles& p, int64_t idx, double out[3]) {
@@ -61,9 +62,11 @@ __device__ __forceinline__ void load_pos(const Particles& p, int64_t idx, double
 
 // minimum image of `ref` (PAPER.md silent; Q3/Q4).  Individually rounded IEEE ops
 // (no FMA contraction) so the integer cell ranges match the oracle bit for bit.
-__device__ __forceinline__ double unwrap1(double x, double ref, double L) {
+__device__ __forceinline__ double unwrap1(double x, double ref, double L, double inv_L) {
     double d = __dsub_rn(x, ref);
-    double q = __ddiv_rn(d, L);
+    // d / L, correctly rounded as in the oracle; when L is a power of two the product with the
+    // (exact) reciprocal is the same number and spares the division's long instruction sequence
+    double q = inv_L != 0.0 ? __dmul_rn(d, inv_L) : __ddiv_rn(d, L);
     double r = rint(q);
     double s = __dmul_rn(L, r);
     return __dsub_rn(x, s);
@@ -189,7 +192,7 @@ __device__ __forceinline__ void load_tet_vertices(const Particles& p, int64_t ce
 #pragma unroll
     for (int v = 1; v < 4; ++v)
 #pragma unroll
-        for (int x = 0; x < 3; ++x) P[v][x] = unwrap1(P[v][x], P[0][x], p.L);
+        for (int x = 0; x < 3; ++x) P[v][x] = unwrap1(P[v][x], P[0][x], p.L, p.inv_L);
 }
 
 // 1/x to about 1 ulp for a normal, non-zero x, without the IEEE division's special-case path:

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
         for (int b = 1; b < 8; ++b)
 #pragma unroll
             for (int x = 0; x < 3; ++x) {
-                C[b][x] = unwrap1(C[b][x], C[0][x], p.L);
+                C[b][x] = unwrap1(C[b][x], C[0][x], p.L, p.inv_L);
                 if (!SCATTER && (b == 1 || b == 2 || b == 4))
                     suspect |= fabs(C[b][x] - C[0][x]) > 0.25 * p.L;
             }
@@ -1031,7 +1031,7 @@ __global__ void __launch_bounds__(256) k_tet_stats(Particles p, double scale, un
             for (int b = 1; b <= 4; b <<= 1) {
                 load_pos(p, corner_index(i, j, k, b, N), c);
 #pragma unroll
-                for (int x = 0; x < 3; ++x) suspect |= fabs(unwrap1(c[x], c0[x], p.L) - c0[x]) > 0.25 * p.L;
+                for (int x = 0; x < 3; ++x) suspect |= fabs(unwrap1(c[x], c0[x], p.L, p.inv_L) - c0[x]) > 0.25 * p.L;
             }
         }
     }
@@ -1146,7 +1146,7 @@ __global__ void __launch_bounds__(128) k_subblock_counts(Particles p, int base_G
         load_pos(p, ((int64_t)ii * N + jj) * N + kk, v);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const double x = unwrap1(v[c], ref[c], p.L);
+            const double x = unwrap1(v[c], ref[c], p.L, p.inv_L);
             lo[c] = fmin(lo[c], x); hi[c] = fmax(hi[c], x);
         }
     }
