@@ -80,6 +80,13 @@ enum {
                                 cell range covers at most this many cells of the tile is class
                                 "small", else "large"; a power of two in [1, 512] (default 8) so
                                 that the classes are unions of the census buckets hist_pair[b] */
+    PSD_OPT_PAIR_RECORDS = 8,  /* binned path.  1 (default): stage A of every (tet, tile) pair (tet
+                                rebuilt from its id, determinant, tile-local vertices, per-row
+                                column ranges of its faces) runs in its own kernel, which writes
+                                144-byte pair records that the deposit kernel reads; the record
+                                buffer holds up to 48 Mi pairs and is refilled slab by slab.
+                                0: the deposit kernel runs stage A itself (no record buffer).
+                                A value > 1 sets the buffer's capacity in pairs (tests).       */
     PSD_OPT_PATCH_RESTRICT = 7  /* psd_deposit_patches, PAPER.md:193 (coarser representations of the
                                 internal nodes).  1 (default): a listed patch whose 8 children are
                                 all listed too is not deposited into; it is filled afterwards by

@@ -13,7 +13,7 @@ import numpy as np
 from . import _build
 
 F32, F64 = 0, 1
-OPT_WEIGHT_MODE, OPT_KERNEL, OPT_COUNTERS, OPT_CHUNK, OPT_CHORD_AXIS, OPT_REFINE_SUBBLOCK, OPT_CLASS_SMALL_CELLS, OPT_PATCH_RESTRICT = 0, 1, 2, 3, 4, 5, 6, 7
+OPT_WEIGHT_MODE, OPT_KERNEL, OPT_COUNTERS, OPT_CHUNK, OPT_CHORD_AXIS, OPT_REFINE_SUBBLOCK, OPT_CLASS_SMALL_CELLS, OPT_PATCH_RESTRICT, OPT_PAIR_RECORDS = 0, 1, 2, 3, 4, 5, 6, 7, 8
 SUBBLOCK_UNIT = 1 << 20
 RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN = 0, 1
 

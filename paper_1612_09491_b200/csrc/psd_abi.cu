@@ -46,11 +46,13 @@ struct psd_ctx {
     Particles part{};
     bool built = false;
     double total_mass = 0.0;
-    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1;
+    int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1,
+        use_records = 1;
+    unsigned long long rec_pairs_max = 48ull << 20;  // capacity of the pair-record buffer (REC_PAIRS_MAX)
     long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 1024;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
-        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families;
+        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families, records, slab_bounds;
     unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
     psd_stats last{};
     bool stats_pending = false;
@@ -87,7 +89,11 @@ int cuda_fail(psd_ctx* c, cudaError_t e, const char* what) {
         if (_e != cudaSuccess) return cuda_fail(ctx, _e, #call);    \
     } while (0)
 
-constexpr int PINNED_WORDS = ST_COUNT + 128 + 2 + psd_ctx::MAX_SLABS + 1;
+// pair records (psd_kernels.cuh, k_pair_records): 13 doubles + 4 u64 + 2 u32 per pair
+constexpr size_t REC_BYTES = 13 * 8 + 4 * 8 + 2 * 4;
+constexpr unsigned long long REC_PAIRS_MAX = 48ull << 20;  // 48 Mi pairs = 6.9 GB
+constexpr int REC_MAX_SLABS = 2048;  // record-buffer slabs of one deposit
+constexpr int PINNED_WORDS = ST_COUNT + 128 + 2 + 2 * (psd_ctx::MAX_SLABS + 1) + 2 * (REC_MAX_SLABS + 2);
 
 int reset_stats(psd_ctx* ctx) {
     CK(ctx->stats.ensure(sizeof(unsigned long long) * ST_COUNT));
@@ -148,6 +154,9 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             const long long bin = (long long)(sl * space.nt / n_slabs) * space.nt * space.nt * N_CLASSES;
             CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + sl, ctx->item_offsets.as<unsigned long long>() + bin,
                                sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+            CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + psd_ctx::MAX_SLABS + 1 + sl,
+                               ctx->tile_offsets.as<unsigned long long>() + bin, sizeof(unsigned long long),
+                               cudaMemcpyDeviceToHost, st));
         }
     }
     CK(cudaStreamSynchronize(st));
@@ -168,7 +177,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                              nullptr, nullptr);
         ctx->launches += 2;
         CK(cudaEventRecord(ctx->ev[3], st));
-        DepositArgs A;
+        DepositArgs A{};
         A.part = ctx->part;
         A.space = space;
         A.pair_ids = ctx->pair_ids.as<unsigned int>();
@@ -188,21 +197,87 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.acc_scale = std::ldexp(1.0, 61 - eu - ec);
             A.acc_inv_scale = std::ldexp(1.0, -(61 - eu - ec));
         }
-        if (n_slabs > 1) {
-            // one launch per slab of x-tiles (items are in tile order); the finished slab of the grid
-            // goes to the host on the copy stream while the next slabs are deposited
-            unsigned long long* ib = ctx->pinned + ST_COUNT + 130;
-            ib[0] = 0; ib[n_slabs] = n_items;
-            const Item* items0 = A.items;
-            const size_t plane = sizeof(double) * (size_t)space.G * space.G;
-            for (int sl = 0; sl < n_slabs; ++sl) {
-                const unsigned int cnt = (unsigned int)(ib[sl + 1] - ib[sl]);
-                if (cnt) {
-                    A.items = items0 + ib[sl];
-                    if (ctx->counters) k_deposit_tiles<true><<<cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
-                    else k_deposit_tiles<false><<<cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+        // ---- launch ranges of work items.  Boundaries (item index, first pair): the slabs of x-tiles
+        // whose part of the grid goes back to the host while later slabs are deposited (host-output
+        // mode), and the slabs of the pair-record buffer (k_pair_records writes the records of a
+        // range, k_deposit_tiles consumes them; the buffer holds rec_cap pairs).
+        struct Bound { unsigned long long item, pair; int x_slab_end; };
+        Bound bounds[psd_ctx::MAX_SLABS + REC_MAX_SLABS + 4];
+        int nb = 0;
+        {
+            const unsigned long long* ib = ctx->pinned + ST_COUNT + 130;
+            const unsigned long long* pb = ib + psd_ctx::MAX_SLABS + 1;
+            bounds[nb++] = Bound{0ull, 0ull, -1};
+            for (int sl = 1; sl < n_slabs; ++sl) bounds[nb++] = Bound{ib[sl], pb[sl], sl - 1};
+            bounds[nb++] = Bound{n_items, n_pairs, n_slabs > 1 ? n_slabs - 1 : -1};
+        }
+        unsigned long long rec_cap = 0;
+        if (ctx->use_records) {
+            const unsigned long long want = n_pairs < ctx->rec_pairs_max ? n_pairs : ctx->rec_pairs_max;
+            if (ctx->records.ensure((size_t)want * REC_BYTES) == cudaSuccess) rec_cap = want;
+            // (no room: the deposit kernel then runs stage A itself)
+        }
+        if (rec_cap && n_pairs > rec_cap) {
+            // cut at multiples of (rec_cap - chunk) pairs: a tiny kernel finds the items, one more
+            // host round trip for them
+            if (rec_cap <= 2ull * ctx->chunk) rec_cap = 0;
+            else {
+                const unsigned long long step = rec_cap - ctx->chunk;
+                const unsigned long long ns = (n_pairs + step - 1) / step;
+                if (ns > (unsigned long long)REC_MAX_SLABS) rec_cap = 0;
+                else {
+                    CK(ctx->slab_bounds.ensure(sizeof(unsigned long long) * 2 * (size_t)(ns + 1)));
+                    k_slab_bounds<<<(unsigned int)((ns + 63) / 64), 64, 0, st>>>(A.items, n_items, n_pairs, step, (int)ns,
+                                                                                ctx->slab_bounds.as<unsigned long long>());
+                    ctx->launches += 1;
+                    unsigned long long* hb = ctx->pinned + ST_COUNT + 130 + 2 * (psd_ctx::MAX_SLABS + 1);
+                    CK(cudaMemcpyAsync(hb, ctx->slab_bounds.p, sizeof(unsigned long long) * 2 * (size_t)ns,
+                                       cudaMemcpyDeviceToHost, st));
+                    CK(cudaStreamSynchronize(st));
+                    // merge (both lists ascend by item)
+                    Bound merged[psd_ctx::MAX_SLABS + REC_MAX_SLABS + 4];
+                    int nm = 0, ia = 0;
+                    unsigned long long s = 1;  // slab 0 starts at item 0, already a boundary
+                    while (ia < nb || s < ns) {
+                        const bool take_a = ia < nb && (s >= ns || bounds[ia].item <= hb[2 * s]);
+                        if (take_a) {
+                            if (s < ns && hb[2 * s] == bounds[ia].item) ++s;
+                            merged[nm++] = bounds[ia++];
+                        } else {
+                            merged[nm++] = Bound{hb[2 * s], hb[2 * s + 1], -1};
+                            ++s;
+                        }
+                    }
+                    nb = nm;
+                    for (int i = 0; i < nb; ++i) bounds[i] = merged[i];
+                }
+            }
+        }
+        if (rec_cap) {
+            char* rb = ctx->records.as<char>();
+            A.rec_stride = (long long)rec_cap;
+            A.rec_g = reinterpret_cast<const double*>(rb);
+            A.rec_rows = reinterpret_cast<const unsigned long long*>(rb + 13 * 8 * rec_cap);
+            A.rec_word = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap);
+            A.rec_cnts = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap + 4 * rec_cap);
+        }
+        const Item* items0 = A.items;
+        const size_t plane = sizeof(double) * (size_t)space.G * space.G;
+        for (int i = 0; i + 1 < nb; ++i) {
+            const unsigned long long cnt = bounds[i + 1].item - bounds[i].item;
+            if (cnt) {
+                A.items = items0 + bounds[i].item;
+                A.rec_pair_begin = bounds[i].pair;
+                if (rec_cap) {
+                    k_pair_records<<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
                     ctx->launches += 1;
                 }
+                if (ctx->counters) k_deposit_tiles<true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                else k_deposit_tiles<false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                ctx->launches += 1;
+            }
+            const int sl = bounds[i + 1].x_slab_end;
+            if (sl >= 0) {  // a slab of x-tiles is complete: its part of the grid goes to the host
                 CK(cudaEventRecord(ctx->slab_ev[sl], st));
                 CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_ev[sl], 0));
                 const size_t x0 = (size_t)(sl * space.nt / n_slabs) * TILE, x1 = (size_t)((sl + 1) * space.nt / n_slabs) * TILE;
@@ -210,6 +285,8 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                    reinterpret_cast<const char*>(space.out) + x0 * plane, (x1 - x0) * plane,
                                    cudaMemcpyDeviceToHost, ctx->copy_stream));
             }
+        }
+        if (n_slabs > 1) {
             CK(cudaEventRecord(ctx->copy_done, ctx->copy_stream));
             CK(cudaEventRecord(ctx->ev[4], st));  // the deposit's own time ends here
             CK(cudaStreamWaitEvent(st, ctx->copy_done, 0));
@@ -219,11 +296,6 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             ctx->binned_last = true;
             return PSD_OK;
         }
-        if (ctx->counters)
-            k_deposit_tiles<true><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
-        else
-            k_deposit_tiles<false><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
-        ctx->launches += 1;
     } else {
         CK(cudaEventRecord(ctx->ev[3], st));
     }
@@ -246,7 +318,7 @@ int run_direct(psd_ctx* ctx, Space space) {
     CK(cudaEventRecord(ctx->ev[1], st));
     CK(cudaEventRecord(ctx->ev[2], st));
     CK(cudaEventRecord(ctx->ev[3], st));
-    DepositArgs A;
+    DepositArgs A{};
     A.part = ctx->part;
     A.space = space;
     A.pair_ids = nullptr;
@@ -309,7 +381,7 @@ void psd_destroy(psd_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->tile_counts, &ctx->cursors, &ctx->tile_offsets, &ctx->item_offsets, &ctx->items,
                       &ctx->pair_ids, &ctx->part_pairs, &ctx->part_items, &ctx->totals, &ctx->stats, &ctx->hist,
-                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families};
+                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families, &ctx->records, &ctx->slab_bounds};
     for (DevBuf* b : bufs) b->release();
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 6; ++i)
@@ -754,6 +826,11 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
             if (iv < 1 || iv > TILE_CELLS || (iv & (iv - 1)))
                 return fail(ctx, PSD_ERR_INVALID_ARG, "class threshold must be a power of two in [1, 512]");
             ctx->class_small = iv; return PSD_OK;
+        case PSD_OPT_PAIR_RECORDS:
+            if (value < 0.0 || value > 4e9) return fail(ctx, PSD_ERR_INVALID_ARG, "pair records: 0, 1 or a capacity in pairs");
+            ctx->use_records = value != 0.0;
+            ctx->rec_pairs_max = value > 1.0 ? (unsigned long long)value : REC_PAIRS_MAX;
+            return PSD_OK;
         case PSD_OPT_PATCH_RESTRICT:
             if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "patch restriction must be 0 or 1");
             ctx->patch_restrict = iv; return PSD_OK;

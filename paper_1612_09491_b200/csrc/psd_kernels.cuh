@@ -379,6 +379,22 @@ __global__ void k_items(const unsigned int* counts, long long n, unsigned int ch
     }
 }
 
+// first work item whose pair list starts at or after s * step pairs, s = 0..ns-1 (the items ascend
+// by `begin`): out[2s] = item index, out[2s+1] = its first pair (n_pairs past the end)
+__global__ void k_slab_bounds(const Item* items, unsigned long long n_items, unsigned long long n_pairs,
+                              unsigned long long step, int ns, unsigned long long* out) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= ns) return;
+    const unsigned long long target = (unsigned long long)s * step;
+    unsigned long long lo = 0, hi = n_items;  // first index with begin >= target
+    while (lo < hi) {
+        const unsigned long long mid = (lo + hi) >> 1;
+        if (items[mid].begin >= target) hi = mid; else lo = mid + 1;
+    }
+    out[2 * s] = lo;
+    out[2 * s + 1] = lo < n_items ? items[lo].begin : n_pairs;
+}
+
 // ---------------------------------------------------------------- a4-a6 binned deposit
 struct DepositArgs {
     Particles part;
@@ -390,6 +406,14 @@ struct DepositArgs {
     int chord_axis;   // -1 adaptive, else 0..2
     unsigned long long* stats;
     double acc_scale, acc_inv_scale;  // fixed-point tile accumulators (PSD_ACC_FIXED): a power of two and its inverse
+    // pair records (k_pair_records -> k_deposit_tiles), structure of arrays with stride rec_stride;
+    // rec_g == nullptr: the deposit kernel runs stage A itself (fused mode)
+    const double* rec_g;              // [13][rec_stride]
+    const unsigned long long* rec_rows;  // [4][rec_stride]
+    const unsigned int* rec_word;     // [rec_stride]
+    const unsigned int* rec_cnts;     // [rec_stride]
+    long long rec_stride;
+    unsigned long long rec_pair_begin;  // first pair (position in pair_ids) of the record buffer
 };
 
 
@@ -482,70 +506,29 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
     }
 }
 
-// One CTA per work item (a chunk of one tile's pair list), an 8^3 fp64 accumulator in shared
-// memory.  Each warp takes 32 pairs at a time:
-//   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
-//            into the warp's slots; per face the rectangle of columns its projection meets.
-//   stage B  the face jobs (slot, face, column) of the 32 slots, face by face, are numbered by a
-//            warp prefix sum of the rectangle sizes, 32 at a time with lane = job: the triangle
-//            against its column in straight-line code (tri_square_clip: parametric clip of the 3
-//            edges, corners by wall ids; no vertex list is edited, so the lanes do not diverge on
-//            the number of walls), projected area and moment, trivial cells.
-//   stage C  the cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
-//            integrals, shares added to the tile (a4-a6).
-// The tile is flushed to global memory with fp64 reductions at the end (a6).
-template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
-    extern __shared__ double smem[];
-    double* acc = smem;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
-    double* wpoly = wtet + 13 * 32;                                                    // [3 * LB_SLOTS][32]
-    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [4][32]
-    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 4 * 32);             // [32]
-    PolyBuf<32> poly{wpoly + lane};
-    // slots 6..9 of the lane's polygon buffer hold the corners of the column's unit square: their
-    // (v, w) never change (the general clip may overwrite slot 6: restored before the next job)
-    poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; poly.at(7, 1) = 1.0; poly.at(7, 2) = 0.0;
-    poly.at(8, 1) = 1.0; poly.at(8, 2) = 1.0; poly.at(9, 1) = 0.0; poly.at(9, 2) = 1.0;
-    bool slot6_dirty = false;
-
-    const Item item = A.items[blockIdx.x];
-    int level, org[3];
-    double* out;
-    long long str[3];
-    tile_geometry(A.space, item.tile, level, org, out, str);
-    const double scale = level_scale(A.space, level);
-    const int Gl = level_G(A.space, level);
-
-    __shared__ unsigned int sh_next;  // next batch of 32 pairs: warps fetch batches as they finish
-    for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
-    if (threadIdx.x == 0) sh_next = 0u;
-    __syncthreads();
-
-    JobCounters cnt = {0, 0, 0, 0};
-
-    for (;;) {
-        unsigned int base = 0;
-        if (lane == 0) base = atomicAdd(&sh_next, 32u);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (base >= item.count) break;
-        // ---- a1: each lane builds one tet of the batch.  The tet is rebuilt from its id for every
-        // periodic image of the tile it meets (almost always one), so that nothing of stage A stays
-        // in registers across stages B and C.
-        const bool have = base + lane < item.count;
-        // the list is taken from its end: the large class first, the small pairs last, so that the
-        // warps of the CTA reach the end-of-item barrier closer together
-        const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - (base + lane))] : 0u;
-        int max_images = 1;
-        for (int img = 0; img < max_images; ++img) {
-            // ---- stage A: slot = lane.  Tile-local vertices, weight, face rectangles.
-            unsigned int cnts = 0u;  // face jobs of this slot, 8 bits per face
-            __syncwarp();
+// ---------------------------------------------------------------- a1-a3 per pair: stage A
+// One (tet, tile) pair, one periodic image of the tile: the tet rebuilt from its id (a1), its
+// determinant and weight, tile-local vertices, chord axis, and per face the columns each row of
+// its rectangle really meets.  Written to the lane's column of three [.][32] blocks:
+//   wt [13][32] doubles  vertex v, coordinate x at row 3 v + x; weight at row 12
+//   wr [4][32]  u64      per face: first row (3 bits), then 7 bits per row: first column, columns
+//   ww [32]     u32      chord axis (2 bits), first / last cell of the tet along it in the tile
+// A tet that goes to one cell whole (inside one cell, or degenerate) is returned as a "special" add.
+struct StageA {
+    unsigned int cnts;   // face jobs, 8 bits per face
+    int my_images;       // periodic images of the tile this tet's range meets
+    bool special;
+    int special_cell;    // cell of the tile, (x*8+y)*8+z
+    double special_val;
+};
+__device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have, const unsigned int id, const int img,
+                                          const int org[3], const int Gl, const double scale, double* wt,
+                                          unsigned long long* wr, unsigned int* ww) {
+    StageA o;
+    o.cnts = 0u; o.my_images = 0; o.special = false; o.special_cell = 0; o.special_val = 0.0;
             Tet t;
             double det = 1.0;
             int nimg[3] = {1, 1, 1}, mlo[3] = {0, 0, 0};
-            int my_images = 0;
             if (have) {
                 double P[4][3];
                 load_tet_vertices(A.part, id / 6, id % 6, P);
@@ -556,10 +539,9 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     mlo[x] = -floor_div(org[x] + TILE - 1 - t.lo[x], Gl);
                     nimg[x] = floor_div(t.hi[x] - org[x], Gl) - mlo[x] + 1;
                 }
-                my_images = nimg[0] * nimg[1] * nimg[2];
+                o.my_images = nimg[0] * nimg[1] * nimg[2];
             }
-            if (img == 0) max_images = __reduce_max_sync(0xffffffffu, my_images);
-            if (img < my_images) {
+            if (img < o.my_images) {
                 int m[3] = {mlo[0] + img % nimg[0], mlo[1] + (img / nimg[0]) % nimg[1],
                             mlo[2] + img / (nimg[0] * nimg[1])};
                 int lo[3], hi[3];
@@ -572,10 +554,10 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
                         gl[v][x] = t.g[v][x] - (double)o;
-                        wtet[(3 * v + x) * 32 + lane] = gl[v][x];
+                        wt[(3 * v + x) * 32] = gl[v][x];
                     }
                 }
-                wtet[12 * 32 + lane] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
+                wt[12 * 32] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
                 int ax = A.chord_axis;
                 if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
                     int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
@@ -593,13 +575,13 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                             c[x] = __double2int_rd(cen) - (org[x] + m[x] * Gl);
                             in = in && c[x] >= 0 && c[x] < TILE;
                         }
-                        if (in) tile_add(&acc[(c[0] * TILE + c[1]) * TILE + c[2]], tile_share(A.mass_per_tet, A.acc_scale));
+                        if (in) { o.special = true; o.special_cell = (c[0] * TILE + c[1]) * TILE + c[2]; o.special_val = A.mass_per_tet; }
                     }
                 } else if (t.lo[0] == t.hi[0] && t.lo[1] == t.hi[1] && t.lo[2] == t.hi[2]) {
                     // a4, tet inside one cell ("trivial cases"): the whole tet goes
                     // to that cell -- m, or its signed volume det/6 in signed-volume mode
-                    tile_add(&acc[(lo[0] * TILE + lo[1]) * TILE + lo[2]],
-                             tile_share(A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0), A.acc_scale));
+                    o.special = true; o.special_cell = (lo[0] * TILE + lo[1]) * TILE + lo[2];
+                    o.special_val = A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0);
                 } else {
                     // per vertex: floor / ceil of (v, w) and ceil of u, read back through the
                     // runtime axis (the lane's own stores above); the faces' rectangles are then
@@ -612,8 +594,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     constexpr double ROW_EPS = 1e-9;
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
-                        const double pu = wtet[(3 * v + ax) * 32 + lane], pv = wtet[(3 * v + av) * 32 + lane];
-                        const double pw = wtet[(3 * v + aw) * 32 + lane];
+                        const double pu = wt[(3 * v + ax) * 32], pv = wt[(3 * v + av) * 32];
+                        const double pw = wt[(3 * v + aw) * 32];
                         fv[v] = __double2int_rd(pv); cvv[v] = __double2int_ru(pv);
                         fw[v] = __double2int_rd(pw); cww[v] = __double2int_ru(pw);
                         cuu[v] = __double2int_ru(pu);
@@ -682,16 +664,142 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                                 llo = ulo; lhi = uhi;
                             }
                         }
-                        cnts |= (unsigned int)c << (8 * f);
-                        wrect[f * 32 + lane] = rows;
+                        o.cnts |= (unsigned int)c << (8 * f);
+                        wr[f * 32] = rows;
                     }
                     rect_written = true;
                 }
                 const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
                 const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
-                if (!rect_written) { wrect[lane] = 0ull; wrect[32 + lane] = 0ull; wrect[64 + lane] = 0ull; wrect[96 + lane] = 0ull; }
-                wword[lane] = (unsigned int)(ax | lou << 2 | hiu << 5);
+                if (!rect_written) { wr[0] = 0ull; wr[32] = 0ull; wr[64] = 0ull; wr[96] = 0ull; }
+                *ww = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
+    return o;
+}
+
+// The pair records of a range of work items: stage A of every pair (image 0), one thread per pair,
+// written field by field (structure of arrays over the record index: the deposit kernel reads
+// them coalesced).  Splitting stage A off keeps the deposit kernel's instruction footprint inside
+// the 32 KB instruction cache (with stage A inlined 18 % of its stall samples were no-instruction).
+// Record index = (pair's position in the item, taken from the item's end) + item.begin - rec_pair_begin.
+constexpr int REC_THREADS = 128;
+__global__ void __launch_bounds__(REC_THREADS) k_pair_records(DepositArgs A) {
+    __shared__ double swt[REC_THREADS / 32][13 * 32];
+    __shared__ unsigned long long swr[REC_THREADS / 32][4 * 32];
+    __shared__ unsigned int sww[REC_THREADS / 32][32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const Item item = A.items[blockIdx.x];
+    int level, org[3];
+    double* out;
+    long long str[3];
+    tile_geometry(A.space, item.tile, level, org, out, str);
+    const double scale = level_scale(A.space, level);
+    const int Gl = level_G(A.space, level);
+    for (unsigned int k0 = 0; k0 < item.count; k0 += REC_THREADS) {
+        const unsigned int k = k0 + threadIdx.x;
+        const bool have = k < item.count;
+        const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - k)] : 0u;
+        const StageA sa = stage_a(A, have, id, 0, org, Gl, scale, &swt[warp][lane], &swr[warp][lane], &sww[warp][lane]);
+        if (have) {
+            const long long r = (long long)(item.begin - A.rec_pair_begin) + k;
+            double* g = const_cast<double*>(A.rec_g);
+#pragma unroll
+            for (int c = 0; c < 12; ++c) g[c * A.rec_stride + r] = swt[warp][c * 32 + lane];
+            g[12 * A.rec_stride + r] = sa.special ? sa.special_val : swt[warp][12 * 32 + lane];
+            unsigned long long* rw = const_cast<unsigned long long*>(A.rec_rows);
+#pragma unroll
+            for (int f = 0; f < 4; ++f) rw[f * A.rec_stride + r] = swr[warp][f * 32 + lane];
+            const_cast<unsigned int*>(A.rec_word)[r] = (sww[warp][lane] & 0xffu) | (unsigned int)sa.special << 8 |
+                                                        (unsigned int)sa.special_cell << 9 |
+                                                        (unsigned int)min(sa.my_images, 16383) << 18;
+            const_cast<unsigned int*>(A.rec_cnts)[r] = sa.cnts;
+        }
+    }
+}
+
+// One CTA per work item (a chunk of one tile's pair list), an 8^3 fp64 accumulator in shared
+// memory.  Each warp takes 32 pairs at a time:
+//   stage A  lane = pair: build the tet (a1), its determinant and weight, tile-local vertices
+//            into the warp's slots; per face the rectangle of columns its projection meets.
+//   stage B  the face jobs (slot, face, column) of the 32 slots, face by face, are numbered by a
+//            warp prefix sum of the rectangle sizes, 32 at a time with lane = job: the triangle
+//            against its column in straight-line code (tri_square_clip: parametric clip of the 3
+//            edges, corners by wall ids; no vertex list is edited, so the lanes do not diverge on
+//            the number of walls), projected area and moment, trivial cells.
+//   stage C  the cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
+//            integrals, shares added to the tile (a4-a6).
+// The tile is flushed to global memory with fp64 reductions at the end (a6).
+template <bool COUNT>
+__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
+    extern __shared__ double smem[];
+    double* acc = smem;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
+    double* wpoly = wtet + 13 * 32;                                                    // [3 * LB_SLOTS][32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [4][32]
+    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 4 * 32);             // [32]
+    PolyBuf<32> poly{wpoly + lane};
+    // slots 6..9 of the lane's polygon buffer hold the corners of the column's unit square: their
+    // (v, w) never change (the general clip may overwrite slot 6: restored before the next job)
+    poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; poly.at(7, 1) = 1.0; poly.at(7, 2) = 0.0;
+    poly.at(8, 1) = 1.0; poly.at(8, 2) = 1.0; poly.at(9, 1) = 0.0; poly.at(9, 2) = 1.0;
+    bool slot6_dirty = false;
+
+    const Item item = A.items[blockIdx.x];
+    int level, org[3];
+    double* out;
+    long long str[3];
+    tile_geometry(A.space, item.tile, level, org, out, str);
+    const double scale = level_scale(A.space, level);
+    const int Gl = level_G(A.space, level);
+
+    __shared__ unsigned int sh_next;  // next batch of 32 pairs: warps fetch batches as they finish
+    for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
+    if (threadIdx.x == 0) sh_next = 0u;
+    __syncthreads();
+
+    JobCounters cnt = {0, 0, 0, 0};
+
+    for (;;) {
+        unsigned int base = 0;
+        if (lane == 0) base = atomicAdd(&sh_next, 32u);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= item.count) break;
+        // ---- a1: each lane builds one tet of the batch.  The tet is rebuilt from its id for every
+        // periodic image of the tile it meets (almost always one), so that nothing of stage A stays
+        // in registers across stages B and C.
+        const bool have = base + lane < item.count;
+        // the list is taken from its end: the large class first, the small pairs last, so that the
+        // warps of the CTA reach the end-of-item barrier closer together
+        const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - (base + lane))] : 0u;
+        int max_images = 1;
+        for (int img = 0; img < max_images; ++img) {
+            // ---- stage A: slot = lane.  From the pair records (k_pair_records ran it for image 0), or
+            // here: the further periodic images of a tile (tiny grids only), and the fused mode
+            __syncwarp();
+            StageA sa;
+            if (A.rec_g != nullptr && img == 0) {
+                sa.cnts = 0u; sa.my_images = 0; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
+                if (have) {
+                    const long long r = (long long)(item.begin - A.rec_pair_begin) + (base + lane);
+#pragma unroll
+                    for (int c = 0; c < 13; ++c) wtet[c * 32 + lane] = A.rec_g[c * A.rec_stride + r];
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) wrect[f * 32 + lane] = A.rec_rows[f * A.rec_stride + r];
+                    const unsigned int word = A.rec_word[r];
+                    wword[lane] = word & 0xffu;
+                    sa.cnts = A.rec_cnts[r];
+                    sa.special = (word >> 8) & 1u;
+                    sa.special_cell = (int)((word >> 9) & 511u);
+                    sa.special_val = wtet[12 * 32 + lane];
+                    sa.my_images = (int)(word >> 18);
+                }
+            } else {
+                sa = stage_a(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
+            }
+            if (sa.special) tile_add(acc + sa.special_cell, tile_share(sa.special_val, A.acc_scale));
+            const unsigned int cnts = sa.cnts;
+            if (img == 0) max_images = __reduce_max_sync(0xffffffffu, sa.my_images);
             // ---- stages B + C for 32 jobs (a lambda with a single call site: its code is large).
             // B: lane = face job (slot, f, cv, cw): clip, area and moment, trivial cells.  C: the
             // cutting planes (polygon, a) of the 32 jobs, numbered by a warp prefix sum, lane = plane;

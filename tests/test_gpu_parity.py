@@ -333,6 +333,32 @@ def test_unwrap_suspects_are_counted_on_both_paths(psd, ctx, kernel):
     assert ctx.psd_get_stats().n_unwrap_suspect == 0
 
 
+@pytest.mark.parametrize("records", [0, 1, 3000, 700])
+def test_pair_record_buffer_modes_agree(psd, ctx, oracle, records):
+    """PSD_OPT_PAIR_RECORDS: stage A in its own kernel writing pair records (default), fused into the
+    deposit kernel (0), and a record buffer far smaller than the pair list (refilled slab by slab,
+    also in the host-output call that streams the grid back in slabs of x-tiles)."""
+    import torch
+    pos = crossing_field(24, 1.5, dtype="float32", stride=4)
+    G = 192
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_set_option(psd.OPT_PAIR_RECORDS, records)
+    ctx.psd_set_option(psd.OPT_CHUNK, 256)
+    ctx.psd_build_tets(to_dev(pos))
+    g = ctx.psd_deposit_uniform(G)
+    assert ctx.psd_get_stats().n_pairs > 20000
+    assert_mass(g.sum())
+    assert_parity(g.cpu().numpy(), ora, what=f"records={records}")
+    hg = torch.full((G, G, G), -1.0, dtype=torch.float64).pin_memory()
+    ctx.psd_deposit_uniform_host(torch.from_numpy(pos).pin_memory(), G, hg)
+    assert_parity(hg.numpy(), ora, what=f"records={records}, host output")
+    # a tiny grid where a tet's range meets a tile in several periodic images
+    pos = crossing_field(12, 2.0)
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 8)
+    ctx.psd_build_tets(to_dev(pos))
+    assert_parity(ctx.psd_deposit_uniform(8).cpu().numpy(), ora, what=f"records={records}, images")
+
+
 def test_error_codes(psd, ctx):
     import torch
     with pytest.raises(psd.PsdError) as e:
