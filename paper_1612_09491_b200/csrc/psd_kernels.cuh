@@ -683,7 +683,10 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
 // the 32 KB instruction cache (with stage A inlined 18 % of its stall samples were no-instruction).
 // Record index = (pair's position in the item, taken from the item's end) + item.begin - rec_pair_begin.
 constexpr int REC_THREADS = 128;
-__global__ void __launch_bounds__(REC_THREADS) k_pair_records(DepositArgs A) {
+#ifndef REC_MIN_CTAS
+#define REC_MIN_CTAS 6
+#endif
+__global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(DepositArgs A) {
     __shared__ double swt[REC_THREADS / 32][13 * 32];
     __shared__ unsigned long long swr[REC_THREADS / 32][4 * 32];
     __shared__ unsigned int sww[REC_THREADS / 32][32];
