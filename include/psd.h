@@ -129,6 +129,8 @@ typedef struct {
     int64_t n_plane_evals;  /* closed-form lattice-plane integrals of a face polygon     */
     int64_t n_cells_written;/* per-face cell shares added to accumulators                */
     int64_t n_restricted_patches; /* psd_deposit_patches: patches filled from their children     */
+    int64_t n_general_clips; /* counters: face jobs the straight-line clip passed to the general
+                               convex clip (a tie within its margin: lattice-aligned input)  */
     /* device pointer to the per-(tile, size class) pair counts of the last binned deposit
        (2 * n_tiles uint32, see psd_get_tile_class_counts) */
     const uint32_t* tile_counts_dev;

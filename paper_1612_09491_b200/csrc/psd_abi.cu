@@ -755,6 +755,7 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
         s.n_face_clips = (int64_t)ctx->pinned[ST_FACE_CLIPS];
         s.n_plane_evals = (int64_t)ctx->pinned[ST_PLANE_CLIPS];
         s.n_cells_written = (int64_t)ctx->pinned[ST_CELLS];
+        s.n_general_clips = (int64_t)ctx->pinned[ST_GENERAL];
         for (int i = 0; i < 64; ++i) {
             s.hist_tet[i] = ctx->pinned[ST_COUNT + i];
             s.hist_pair[i] = ctx->pinned[ST_COUNT + 64 + i];

@@ -353,7 +353,7 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
 }
 
 struct JobCounters {
-    unsigned int jobs, face_clips, plane_evals, cells;
+    unsigned int jobs, face_clips, plane_evals, cells, general;
 };
 
 // faces of tet (0,1,2,3) with outward orientation when det > 0: (1,2,3) (0,3,2) (0,1,3) (0,2,1)

@@ -46,7 +46,7 @@ constexpr int N_CLASSES = 2;
 constexpr long long CLASS_SMALL_MAX_CELLS = 8;  // default of PSD_OPT_CLASS_SMALL_CELLS
 
 enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
-       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_COUNT };
+       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_GENERAL, ST_COUNT };
 
 // ---------------------------------------------------------------- validation of positions
 __global__ void k_validate(Particles p, unsigned long long* stats) {
@@ -761,7 +761,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
     if (threadIdx.x == 0) sh_next = 0u;
     __syncthreads();
 
-    JobCounters cnt = {0, 0, 0, 0};
+    JobCounters cnt = {0, 0, 0, 0, 0};
 
     for (;;) {
         unsigned int base = 0;
@@ -837,6 +837,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         for (int i = 0; i < 3; ++i) { poly.at(i, 0) = U[i]; poly.at(i, 1) = V[i]; poly.at(i, 2) = W[i]; }
                         fc = face_clip_general(wpoly + lane);
                         slot6_dirty = true;
+                        if (COUNT) cnt.general++;
                     } else {
                         fc = poly_area_moment<32>(poly, lb.order, lb.n);
                         if (lb.sign < 0) f_w = -f_w;  // clockwise triangle: the polygon is its mirror image
@@ -983,6 +984,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
             atomicAdd(&A.stats[ST_PLANE_CLIPS], (unsigned long long)c);
             atomicAdd(&A.stats[ST_CELLS], (unsigned long long)d);
         }
+        const unsigned int e = __reduce_add_sync(0xffffffffu, cnt.general);
+        if (lane == 0 && e) atomicAdd(&A.stats[ST_GENERAL], (unsigned long long)e);
     }
 }
 
@@ -1002,7 +1005,7 @@ __global__ void __launch_bounds__(DIR_THREADS) k_deposit_direct(DepositArgs A) {
     PolyBuf<32> poly{ts + 12 * 32};
     const int64_t ntet = (int64_t)6 * A.part.N * A.part.N * A.part.N;
     int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    JobCounters cnt = {0, 0, 0, 0};
+    JobCounters cnt = {0, 0, 0, 0, 0};
     if (id < ntet) {
         const Space& s = A.space;
         const int G = s.G;
