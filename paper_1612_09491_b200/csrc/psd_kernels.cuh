@@ -917,27 +917,21 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 }
                 __syncwarp();
             };
-            // ---- the face jobs (slot, face, column) of the 32 slots, face by face, numbered by a warp
-            // prefix sum of the rectangle sizes; one loop with a single call site of run_jobs
+            // ---- the face jobs (slot, face, row, column) of the 32 slots, numbered by ONE warp prefix
+            // sum of the slots' job counts (all four faces together: one partly filled pass per batch,
+            // not one per face); a loop with a single call site of run_jobs
             __syncwarp();
-            int f = -1, jb = 0, total = 0, pre = 0;
+            const int njobs = (int)((cnts & 255u) + ((cnts >> 8) & 255u) + ((cnts >> 16) & 255u) + (cnts >> 24));
+            int pre = njobs;
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, pre, o);
+                if (lane >= o) pre += y;
+            }
+            const int total = __shfl_sync(0xffffffffu, pre, 31);
+            pre -= njobs;
 #pragma unroll 1
-            for (;;) {
-                if (jb >= total) {  // next face: exclusive prefix of its job counts over the 32 slots
-                    if (++f == 4) break;
-                    const int njobs = (cnts >> (8 * f)) & 255;
-                    pre = njobs;
-                    for (int o = 1; o < 32; o <<= 1) {
-                        int y = __shfl_up_sync(0xffffffffu, pre, o);
-                        if (lane >= o) pre += y;
-                    }
-                    total = __shfl_sync(0xffffffffu, pre, 31);
-                    pre -= njobs;
-                    jb = 0;
-                    continue;
-                }
+            for (int jb = 0; jb < total; jb += 32) {
                 const int job = jb + lane;
-                jb += 32;
                 int slot = 0;  // largest slot with pre[slot] <= job
 #pragma unroll
                 for (int step = 16; step; step >>= 1) {
@@ -945,12 +939,20 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     if (probe <= job) slot += step;
                 }
                 const int spre = __shfl_sync(0xffffffffu, pre, slot);
-                int cv = 0, cw = 0;
+                const unsigned int scnt = __shfl_sync(0xffffffffu, cnts, slot);
+                int cv = 0, cw = 0, f = 0;
                 const bool act = job < total;
                 if (act) {
-                    // decode (slot, row, column): bits 0..2 of the face's word = first row, then 7 bits
-                    // per row = first column (3) and number of columns (4)
+                    // decode (face, row, column): the slot's four face counts, then bits 0..2 of the
+                    // face's word = first row, then 7 bits per row = first column (3), columns (4)
                     int local = job - spre;
+                    unsigned int sc = scnt;
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        const int n = (int)(sc & 255u);
+                        if (local < n) break;
+                        local -= n; ++f; sc >>= 8;
+                    }
                     unsigned long long rw = wrect[f * 32 + slot];
                     cv = (int)(rw & 7ull);
                     rw >>= 3;
