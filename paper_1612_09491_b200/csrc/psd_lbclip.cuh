@@ -62,13 +62,13 @@ __host__ __device__ __forceinline__ LBPiece lb_edge(double va, double wa, double
     p.win = ev ? (upv ? 3 : 1) : (upw ? 0 : 2);
     p.wout = xv ? (upv ? 1 : 3) : (upw ? 2 : 0);
     // ties: the edge's line through a corner of the square, or the edge grazing the square
-    p.amb = fabs(tev - tew) <= PSD_LB_TOL || fabs(txv - txw) <= PSD_LB_TOL;
+    p.amb = (fabs(tev - tew) <= PSD_LB_TOL) | (fabs(txv - txw) <= PSD_LB_TOL);
     if (a_in) { t0 = 0.0; p.win = -1; }
     if (b_in) { t1 = 1.0; p.wout = -1; }
     t0 = t0 < 0.0 ? 0.0 : t0;
     t1 = t1 > 1.0 ? 1.0 : t1;
     p.ok = t0 < t1;
-    p.amb = p.amb || fabs(t1 - t0) <= PSD_LB_TOL;
+    p.amb = p.amb | (fabs(t1 - t0) <= PSD_LB_TOL);
     p.t0 = t0; p.t1 = t1;
     return p;
 }
@@ -101,7 +101,7 @@ __host__ __device__ __forceinline__ LBResult tri_square_clip(PolyBuf<S> q, const
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         v[i] = fma(ms, V[i], mo);
-        in[i] = v[i] >= 0.0 && v[i] <= 1.0 && W[i] >= 0.0 && W[i] <= 1.0;
+        in[i] = (v[i] >= 0.0) & (v[i] <= 1.0) & (W[i] >= 0.0) & (W[i] <= 1.0);
     }
     LBPiece p[3];
     double dv[3], dw[3], du[3];
@@ -154,7 +154,7 @@ __host__ __device__ __forceinline__ LBResult tri_square_clip(PolyBuf<S> q, const
         }
         // the next piece: it starts at this edge's end vertex, or enters through a wall
         const int kin = p[b].ok ? p[b].win : (p[c].ok ? p[c].win : p[e].win);
-        bad = bad || (ok && (endv ? !(p[b].ok && p[b].win < 0) : kin < 0));
+        bad = bad | (ok & (endv ? !(p[b].ok & (p[b].win < 0)) : (kin < 0)));
         const int cnt = (ok && !endv) ? ((kin - p[e].wout) & 3) : 0;
         // corners after wall wout, counter-clockwise: slots 6 + (wout + 1 .. wout + cnt) mod 4
         const unsigned cwd = (0x98769876u >> (4 * ((p[e].wout + 1) & 3))) & ((1u << (4 * cnt)) - 1u);
