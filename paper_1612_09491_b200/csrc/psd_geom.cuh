@@ -308,6 +308,9 @@ __device__ __forceinline__ void clip_wall(PolyBuf<S> q, PolyRef& r, int wall) {
 // lies inside Q and every height is >= 0: a sum of same-signed terms, no cancellation.
 // Returns 6 R (signed like the polygon's orientation).
 template <int S>
+__device__ __forceinline__ double plane_integral6_mask(PolyBuf<S> q, unsigned order, int n, double a, unsigned mask);
+
+template <int S>
 __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, int n, double a) {
     unsigned mask = 0;
 #pragma unroll
@@ -315,6 +318,21 @@ __device__ __forceinline__ double plane_integral6(PolyBuf<S> q, unsigned order, 
         if (i >= n) break;
         mask |= (unsigned)(q.at(slot_of(order, i), 0) >= a) << i;
     }
+    return plane_integral6_mask<S>(q, order, n, a, mask);
+}
+
+// Vertex i is at or above the lattice plane a  <=>  floor(u_i) >= a: with the floors of the
+// polygon's vertex heights packed one nibble each (clamped to 0..8) the inside mask of a plane
+// 1..8 is one add and a bit gather, no loads; plane 0 takes the mask of the vertices below 0.
+__device__ __forceinline__ unsigned plane_mask_from_floors(unsigned floors, unsigned below0, int n, int a) {
+    const unsigned full = (1u << n) - 1u;
+    if (a == 0) return full & ~below0;  // plane 0: every vertex that is not below the tile
+    return gather_nibble_bit(floors + (unsigned)(8 - a) * 0x01111111u, 3) & full;
+}
+
+// the integral proper, inside-mask given (bit i: vertex i has u >= a)
+template <int S>
+__device__ __forceinline__ double plane_integral6_mask(PolyBuf<S> q, unsigned order, int n, double a, unsigned mask) {
     const unsigned full = (1u << n) - 1u;
     if (mask == 0 || mask == full) return 0.0;  // not a cutting plane (caller excludes this)
     int i_out, i_in;
@@ -367,6 +385,8 @@ struct FaceClip {
     int n;            // 0: empty
     double A, M1;     // signed projected area of Q, first moment integral of u over Q
     int ifl, ice;     // floor of the lowest, ceil of the highest vertex height
+    unsigned floors;  // nibble i = floor of vertex i's height, clamped to 0..8 (plane_mask_from_floors)
+    unsigned below0;  // bit i = vertex i's height is below 0
 };
 
 // q holds the face triangle in slots 0..2: (u, v, w) with v, w relative to the column's lower
@@ -392,12 +412,15 @@ __device__ __forceinline__ unsigned tri_outcodes(PolyBuf<S> q, unsigned& all_in,
 template <int S>
 __device__ __forceinline__ FaceClip poly_area_moment(PolyBuf<S> q, unsigned order, int n) {
     FaceClip fc;
-    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0; fc.floors = 0; fc.below0 = 0;
     if (n < 3) return fc;
     const int s0 = slot_of(order, 0), s1 = slot_of(order, 1);
     const double u0 = q.at(s0, 0), v0 = q.at(s0, 1), w0 = q.at(s0, 2);
     double lu = q.at(s1, 0), lv = q.at(s1, 1) - v0, lw = q.at(s1, 2) - w0;
-    int ifl = min(__double2int_rd(u0), __double2int_rd(lu)), ice = max(__double2int_ru(u0), __double2int_ru(lu));
+    const int f0 = __double2int_rd(u0), f1 = __double2int_rd(lu);
+    int ifl = min(f0, f1), ice = max(__double2int_ru(u0), __double2int_ru(lu));
+    unsigned floors = (unsigned)min(max(f0, 0), 8) | (unsigned)min(max(f1, 0), 8) << 4;
+    unsigned below0 = (unsigned)(f0 < 0) | (unsigned)(f1 < 0) << 1;
     double A2 = 0.0, M6 = 0.0;
 #pragma unroll
     for (int i = 2; i < POLY_CAP; ++i) {
@@ -407,10 +430,13 @@ __device__ __forceinline__ FaceClip poly_area_moment(PolyBuf<S> q, unsigned orde
         const double cr = lv * cw - lw * cv;
         A2 += cr;
         M6 = fma(cr, u0 + lu + cu, M6);
-        ifl = min(ifl, __double2int_rd(cu)); ice = max(ice, __double2int_ru(cu));
+        const int fi = __double2int_rd(cu);
+        ifl = min(ifl, fi); ice = max(ice, __double2int_ru(cu));
+        floors |= (unsigned)min(max(fi, 0), 8) << (4 * i);
+        below0 |= (unsigned)(fi < 0) << i;
         lu = cu; lv = cv; lw = cw;
     }
-    fc.order = order; fc.n = n;
+    fc.order = order; fc.n = n; fc.floors = floors; fc.below0 = below0;
     fc.A = 0.5 * A2; fc.M1 = M6 * (1.0 / 6.0);
     fc.ifl = ifl; fc.ice = ice;
     return fc;
@@ -430,7 +456,7 @@ __device__ __forceinline__ FaceClip face_clip(PolyBuf<S> q) {
 template <int S, bool WALLS_UNROLLED>
 __device__ __forceinline__ FaceClip face_clip_oc(PolyBuf<S> q, unsigned oc, unsigned all_in, unsigned any_in) {
     FaceClip fc;
-    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0;
+    fc.n = 0; fc.order = 0; fc.A = fc.M1 = 0.0; fc.ifl = fc.ice = 0; fc.floors = 0; fc.below0 = 0;
     if (any_in != 15u) return fc;  // all three vertices outside one wall
     PolyRef r{0x210u, oc, 3, 3};
     unsigned pending = all_in ^ 15u;

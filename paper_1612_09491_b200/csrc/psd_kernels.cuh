@@ -808,7 +808,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
             // cutting planes (polygon, a) of the 32 jobs, numbered by a warp prefix sum, lane = plane;
             // the kept part above the plane is integrated in closed form; +R to cell a, -R to a-1.
             auto run_jobs = [&](const bool act, const int slot, const int f, const int cv, const int cw) {
-                unsigned int f_order = 0, f_info = 0;
+                unsigned int f_order = 0, f_info = 0, f_floors = 0;
                 int f_afirst = 0, k = 0;
                 double f_w = 0.0;
                 if (act) {
@@ -875,9 +875,10 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         }
                         k = max(fr.a_last - fr.a_first + 1, 0);
                         f_order = fc.order;
+                        f_floors = fc.floors;
                         f_afirst = fr.a_first;
                         f_info = (unsigned)colofs | (unsigned)ax << 9 | (unsigned)c_lo << 11 | (unsigned)c_hi << 14 |
-                                 (unsigned)fc.n << 17;
+                                 (unsigned)fc.n << 17 | fc.below0 << 20;
                     }
                 }
                 __syncwarp();
@@ -899,6 +900,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                     const int s_pre = __shfl_sync(0xffffffffu, pre2, src);
                     const unsigned int s_order = __shfl_sync(0xffffffffu, f_order, src);
                     const unsigned int s_info = __shfl_sync(0xffffffffu, f_info, src);
+                    const unsigned int s_floors = __shfl_sync(0xffffffffu, f_floors, src);
                     const int s_afirst = __shfl_sync(0xffffffffu, f_afirst, src);
                     const double s_w = __shfl_sync(0xffffffffu, f_w, src);
                     if (e < total2) {
@@ -907,7 +909,8 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         const int c_lo = (s_info >> 11) & 7, c_hi = (s_info >> 14) & 7, n = (s_info >> 17) & 7;
                         const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1);
                         PolyBuf<32> qs{wpoly + src};
-                        const double R = plane_integral6<32>(qs, s_order, n, (double)a) * (1.0 / 6.0) * s_w;
+                        const double R = plane_integral6_mask<32>(qs, s_order, n, (double)a, plane_mask_from_floors(s_floors, (s_info >> 20) & 127u, n, a)) *
+                                         (1.0 / 6.0) * s_w;
                         if (COUNT) cnt.plane_evals++;
                         if (R != 0.0) {
                             if (a <= c_hi) { tile_add(acc + colofs + a * su, tile_share(R, A.acc_scale)); if (COUNT) cnt.cells++; }
