@@ -64,7 +64,7 @@ enum {
                                 1: direct path (one thread per tet, global atomics).           */
     PSD_OPT_COUNTERS = 2,    /* 1: also count face jobs / non-empty clips / plane integrals / cell
                                 shares written during deposits (slower; for the work model).    */
-    PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 1024) */
+    PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 2048) */
     PSD_OPT_CHORD_AXIS = 4,  /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
     PSD_OPT_REFINE_SUBBLOCK = 5 /* census used by psd_refine_patches.  0 (default): every tet is
                                 counted.  B in 1..64: the paper's memory-lean

@@ -50,7 +50,7 @@ struct psd_ctx {
         use_records = 1;
     unsigned long long rec_pairs_max = 48ull << 20;  // capacity of the pair-record buffer (REC_PAIRS_MAX)
     long long class_small = CLASS_SMALL_MAX_CELLS;
-    unsigned int chunk = 1024;
+    unsigned int chunk = 2048;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
         totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families, records, slab_bounds;
     unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
