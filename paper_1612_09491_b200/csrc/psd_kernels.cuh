@@ -1,9 +1,12 @@
 // psd_kernels.cuh -- kernels of the deposit path (sm_100a).  Steps:
-//   a1 tet generation        load_tet_vertices, inlined in k_census / k_deposit_* (nothing stored per tet)
+//   a1 tet generation        load_tet_vertices, inlined where a tet is needed (nothing stored per tet)
 //   a2 AABB + census         k_census<false> (pair counts per (tile, size class), histograms)
 //   a3 bin / sort            k_scan_* + k_census<true> (counting sort of tet ids by tile and class) + k_items
+//   a3' per-pair stage A     stage_a / k_pair_records (tile-local vertices, weight, per-row column
+//                            ranges of the faces -> 144-byte pair records), k_slab_bounds
 //   a4-a6 classify, clip, accumulate, flush    k_deposit_tiles (binned) / k_deposit_direct
-//   a7 patch path            the same kernels with Space::patch_mode = 1, k_patch_counts
+//   a7 patch path            the same kernels with Space::patch_mode = 1, k_patch_counts,
+//                            k_subblock_counts, k_restrict
 #pragma once
 #include "psd_geom.cuh"
 #include "psd_lbclip.cuh"
