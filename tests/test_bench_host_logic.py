@@ -85,3 +85,17 @@ def test_roofline_traffic_comes_from_the_committed_capture():
     v = bench.read_ncu_traffic("cfg1_128_256", "k_deposit_tiles")
     assert isinstance(v, int) and v > 100e6
     assert bench.read_ncu_traffic("no_such_workload", "k_deposit_tiles") is None
+    # the headline workload and the patch config have captures too (sums over the record slabs)
+    for w in ("cfg4_512_1024", "cfg3_256_patches", "cfg2_256_512"):
+        assert bench.read_ncu_traffic(w, "k_deposit_tiles") > bench.read_ncu_value(w, "k_deposit_tiles") > 1e9
+        assert bench.read_ncu_fp64_flops(w) > 1e11
+    assert bench.read_ncu_fp64_flops("no_such_workload") is None
+
+
+def test_strided_oracle_sample_covers_the_lattice():
+    import bench
+    r = bench.strided_ranges(512 ** 3, 2_500_000)
+    assert len(r) == 64 and r[0][0] == 0 and r[-1][0] > 0.98 * 512 ** 3 * 63 / 64
+    assert all(b < e <= 512 ** 3 for b, e in r) and all(r[i][1] <= r[i + 1][0] for i in range(63))
+    assert sum(e - b for b, e in r) <= 2_500_000
+    assert bench.strided_ranges(10, 100) == [(i, i + 1) for i in range(10)]
