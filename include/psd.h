@@ -115,6 +115,7 @@ typedef struct {
     int64_t n_work_items; /* chunks of pair lists scheduled                              */
     int64_t sum_cells;    /* sum over tets of AABB cells (candidate cells)               */
     int64_t max_cells;    /* largest AABB                                                */
+    int64_t max_extent;   /* largest cell range of a tet along one axis (binned path)    */
     int64_t n_inverted;   /* tets with negative determinant                */
     int64_t n_degenerate; /* tets with determinant exactly 0                             */
     int64_t n_unwrap_suspect; /* Lagrangian cells with an unwrapped edge longer than L/4: the

@@ -38,7 +38,7 @@ class PsdPatch(C.Structure):
 class PsdStats(C.Structure):
     _fields_ = [
         ("n_tets", C.c_int64), ("n_tiles", C.c_int64), ("n_pairs", C.c_int64),
-        ("n_work_items", C.c_int64), ("sum_cells", C.c_int64), ("max_cells", C.c_int64),
+        ("n_work_items", C.c_int64), ("sum_cells", C.c_int64), ("max_cells", C.c_int64), ("max_extent", C.c_int64),
         ("n_inverted", C.c_int64), ("n_degenerate", C.c_int64), ("n_unwrap_suspect", C.c_int64),
         ("n_nonfinite", C.c_int64),
         ("hist_tet", C.c_uint64 * 64), ("hist_pair", C.c_uint64 * 64),

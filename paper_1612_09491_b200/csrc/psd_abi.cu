@@ -159,8 +159,11 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                cudaMemcpyDeviceToHost, st));
         }
     }
+    CK(cudaMemcpyAsync(ctx->pinned + ST_MAX_EXTENT, ctx->stats.as<unsigned long long>() + ST_MAX_EXTENT,
+                       sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     const unsigned long long n_pairs = ctx->pinned[ST_COUNT + 128], n_items = ctx->pinned[ST_COUNT + 129];
+    const unsigned long long max_extent = ctx->pinned[ST_MAX_EXTENT];  // largest cell range of a tet along an axis (level 0)
     ctx->last.n_pairs = (int64_t)n_pairs;
     ctx->last.n_work_items = (int64_t)n_items;
     ctx->last.n_tiles = n_tiles;
@@ -261,6 +264,10 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.rec_word = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap);
             A.rec_cnts = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap + 4 * rec_cap);
         }
+        // The records-only deposit kernel needs every pair to meet its tile in one periodic image:
+        // true when the largest cell range of a tet plus a tile fits the (coarsest) grid.
+        const long long g_min = space.patch_mode ? space.base_G : space.G;
+        const bool rec_only = rec_cap != 0 && (long long)max_extent + 2 + TILE < g_min;
         const Item* items0 = A.items;
         const size_t plane = sizeof(double) * (size_t)space.G * space.G;
         for (int i = 0; i + 1 < nb; ++i) {
@@ -272,8 +279,13 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                     k_pair_records<<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
                     ctx->launches += 1;
                 }
-                if (ctx->counters) k_deposit_tiles<true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
-                else k_deposit_tiles<false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                if (rec_only) {
+                    if (ctx->counters) k_deposit_tiles<true, true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
+                    else k_deposit_tiles<false, true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
+                } else {
+                    if (ctx->counters) k_deposit_tiles<true, false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                    else k_deposit_tiles<false, false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+                }
                 ctx->launches += 1;
             }
             const int sl = bounds[i + 1].x_slab_end;
@@ -364,9 +376,13 @@ int psd_create(psd_ctx** out, int device, void* cuda_stream) {
         e = cudaEventCreateWithFlags(&ctx->slab_ev[i], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->copy_done, cudaEventDisableTiming);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_deposit_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
+        e = cudaFuncSetAttribute(k_deposit_tiles<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_deposit_tiles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
+        e = cudaFuncSetAttribute(k_deposit_tiles<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_tiles<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_tiles<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
     if (e != cudaSuccess) {
         psd_destroy(ctx);
         return PSD_ERR_CUDA;
@@ -748,6 +764,7 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
         psd_stats& s = ctx->last;
         s.sum_cells = (int64_t)ctx->pinned[ST_SUM_CELLS];
         s.max_cells = (int64_t)ctx->pinned[ST_MAX_CELLS];
+        s.max_extent = (int64_t)ctx->pinned[ST_MAX_EXTENT];
         s.n_inverted = (int64_t)ctx->pinned[ST_INVERTED];
         s.n_degenerate = (int64_t)ctx->pinned[ST_DEGENERATE];
         s.n_unwrap_suspect = (int64_t)ctx->pinned[ST_UNWRAP];

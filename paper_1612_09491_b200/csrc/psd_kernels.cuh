@@ -49,7 +49,7 @@ constexpr int N_CLASSES = 2;
 constexpr long long CLASS_SMALL_MAX_CELLS = 8;  // default of PSD_OPT_CLASS_SMALL_CELLS
 
 enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
-       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_GENERAL, ST_COUNT };
+       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_GENERAL, ST_MAX_EXTENT, ST_COUNT };
 
 // ---------------------------------------------------------------- validation of positions
 __global__ void k_validate(Particles p, unsigned long long* stats) {
@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
     int64_t cell = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     // statistics are summed per thread over its 6 tets, then per warp, then one shared atomic each
     unsigned long long t_sum = 0, t_max = 0;
-    unsigned int t_inv = 0, t_deg = 0, t_pairs = 0, t_suspect = 0;
+    unsigned int t_inv = 0, t_deg = 0, t_pairs = 0, t_suspect = 0, t_ext = 0;
     if (cell < ncell) {
         int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((int64_t)N * N));
         double C[8][3];
@@ -194,6 +194,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
                                    (t.hi[2] - t.lo[2] + 1);
                     t_sum += (unsigned long long)nc;
                     t_max = (unsigned long long)nc > t_max ? (unsigned long long)nc : t_max;
+                    t_ext = max(t_ext, (unsigned int)max(max(t.hi[0] - t.lo[0], t.hi[1] - t.lo[1]), t.hi[2] - t.lo[2]) + 1u);
                     atomicAdd(&sh_hist[0][bit_width_u64((unsigned long long)(nc - 1))], 1u);
                     double det = tet_det_sign(t.g);
                     t_inv += det < 0.0;
@@ -233,7 +234,9 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
         t_deg = __reduce_add_sync(0xffffffffu, t_deg);
         t_pairs = __reduce_add_sync(0xffffffffu, t_pairs);
         t_suspect = __reduce_add_sync(0xffffffffu, t_suspect);
+        t_ext = __reduce_max_sync(0xffffffffu, t_ext);
         if ((threadIdx.x & 31) == 0) {
+            atomicMax(&sh_stat[ST_MAX_EXTENT], (unsigned long long)t_ext);
             atomicAdd(&sh_stat[ST_SUM_CELLS], t_sum);
             atomicMax(&sh_stat[ST_MAX_CELLS], t_max);
             if (t_inv) atomicAdd(&sh_stat[ST_INVERTED], (unsigned long long)t_inv);
@@ -247,7 +250,7 @@ __global__ void __launch_bounds__(256) k_census(Particles p, Space s, unsigned i
             if (v) atomicAdd(&hist[i], (unsigned long long)v);
         }
         if (threadIdx.x < ST_COUNT && sh_stat[threadIdx.x]) {
-            if (threadIdx.x == ST_MAX_CELLS) atomicMax(&stats[ST_MAX_CELLS], sh_stat[ST_MAX_CELLS]);
+            if (threadIdx.x == ST_MAX_CELLS || threadIdx.x == ST_MAX_EXTENT) atomicMax(&stats[threadIdx.x], sh_stat[threadIdx.x]);
             else atomicAdd(&stats[threadIdx.x], sh_stat[threadIdx.x]);
         }
     }
@@ -481,6 +484,13 @@ constexpr int DEP_THREADS = DEP_WARPS * 32;
 // [3*LB_SLOTS][32], per-face row ranges [4][32] (u64), slot words [32] (u32)
 constexpr int WARP_SCRATCH = (13 + 3 * LB_SLOTS) * 32 + 4 * 32 + 16;
 constexpr int DEP_SMEM_BYTES = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH) * 8;
+// the records-only kernel (k_deposit_tiles<COUNT, true>) reads the slots' data straight from the
+// pair records (L1): its per-warp scratch is the polygon buffer alone -> 6 CTAs per SM instead of 4
+constexpr int WARP_SCRATCH_REC = 3 * LB_SLOTS * 32;
+constexpr int DEP_SMEM_BYTES_REC = (TILE_CELLS + DEP_WARPS * WARP_SCRATCH_REC) * 8;
+#ifndef DEP_MIN_CTAS_REC
+#define DEP_MIN_CTAS_REC 6
+#endif
 
 // The general convex clip (clip_wall) of one face job, for the jobs the straight-line clip
 // reports as ambiguous (lattice-aligned input): kept out of line, it runs rarely.
@@ -735,15 +745,17 @@ __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(Depo
 //   stage C  the cutting planes of the 32 polygons re-numbered over the lanes, closed-form plane
 //            integrals, shares added to the tile (a4-a6).
 // The tile is flushed to global memory with fp64 reductions at the end (a6).
-template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
+// REC = true: every pair has a record and meets its tile in one periodic image only (the host
+// checks the largest cell range against the grid): no stage A code, no slot staging in shared memory.
+template <bool COUNT, bool REC>
+__global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_CTAS) k_deposit_tiles(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* wtet = smem + TILE_CELLS + warp * WARP_SCRATCH;                           // [13][32]
-    double* wpoly = wtet + 13 * 32;                                                    // [3 * LB_SLOTS][32]
-    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [4][32]
-    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 4 * 32);             // [32]
+    double* wtet = smem + TILE_CELLS + warp * (REC ? WARP_SCRATCH_REC : WARP_SCRATCH);  // [13][32] (not REC)
+    double* wpoly = REC ? wtet : wtet + 13 * 32;                                       // [3 * LB_SLOTS][32]
+    unsigned long long* wrect = reinterpret_cast<unsigned long long*>(wpoly + 3 * LB_SLOTS * 32);  // [4][32] (not REC)
+    unsigned int* wword = reinterpret_cast<unsigned int*>(wrect + 4 * 32);             // [32] (not REC)
     PolyBuf<32> poly{wpoly + lane};
     // slots 6..9 of the lane's polygon buffer hold the corners of the column's unit square: their
     // (v, w) never change (the general clip may overwrite slot 6: restored before the next job)
@@ -777,14 +789,25 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
         const bool have = base + lane < item.count;
         // the list is taken from its end: the large class first, the small pairs last, so that the
         // warps of the CTA reach the end-of-item barrier closer together
-        const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - (base + lane))] : 0u;
+        const unsigned int id = (!REC && have) ? A.pair_ids[item.begin + (item.count - 1u - (base + lane))] : 0u;
+        // record of slot 0 of this batch (REC: the slots' data is read from the records where it is used)
+        const long long rb = (long long)(item.begin - A.rec_pair_begin) + base;
         int max_images = 1;
         for (int img = 0; img < max_images; ++img) {
             // ---- stage A: slot = lane.  From the pair records (k_pair_records ran it for image 0), or
             // here: the further periodic images of a tile (tiny grids only), and the fused mode
             __syncwarp();
             StageA sa;
-            if (A.rec_g != nullptr && img == 0) {
+            if (REC) {
+                sa.cnts = 0u; sa.my_images = 1; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
+                if (have) {
+                    const unsigned int word = __ldg(A.rec_word + rb + lane);
+                    sa.cnts = __ldg(A.rec_cnts + rb + lane);
+                    sa.special = (word >> 8) & 1u;
+                    sa.special_cell = (int)((word >> 9) & 511u);
+                    if (sa.special) sa.special_val = __ldg(A.rec_g + 12 * A.rec_stride + rb + lane);
+                }
+            } else if (A.rec_g != nullptr && img == 0) {
                 sa.cnts = 0u; sa.my_images = 0; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
                 if (have) {
                     const long long r = (long long)(item.begin - A.rec_pair_begin) + (base + lane);
@@ -805,7 +828,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
             }
             if (sa.special) tile_add(acc + sa.special_cell, tile_share(sa.special_val, A.acc_scale));
             const unsigned int cnts = sa.cnts;
-            if (img == 0) max_images = __reduce_max_sync(0xffffffffu, sa.my_images);
+            if (!REC && img == 0) max_images = __reduce_max_sync(0xffffffffu, sa.my_images);
             // ---- stages B + C for 32 jobs (a lambda with a single call site: its code is large).
             // B: lane = face job (slot, f, cv, cw): clip, area and moment, trivial cells.  C: the
             // cutting planes (polygon, a) of the 32 jobs, numbered by a warp prefix sum, lane = plane;
@@ -816,22 +839,29 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                 double f_w = 0.0;
                 if (act) {
                     if (COUNT) cnt.jobs++;
-                    const unsigned int word = wword[slot];
+                    const unsigned int word = REC ? __ldg(A.rec_word + rb + slot) : wword[slot];
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
                     // the face triangle, column-local
                     const double* ts = wtet + slot;
+                    const double* tr = A.rec_g + rb + slot;   // REC: the slot's record, row c at tr[c * rec_stride]
                     const unsigned int fv = FACE_TABLE >> (6 * f);
                     const double ov = (double)cv, ow = (double)cw;
                     double U[3], V[3], W[3];
 #pragma unroll
                     for (int i = 0; i < 3; ++i) {
                         const int vi = (fv >> (2 * i)) & 3;
-                        U[i] = ts[(3 * vi + ax) * 32];
-                        V[i] = ts[(3 * vi + av) * 32] - ov;
-                        W[i] = ts[(3 * vi + aw) * 32] - ow;
+                        if (REC) {
+                            U[i] = __ldg(tr + (3 * vi + ax) * A.rec_stride);
+                            V[i] = __ldg(tr + (3 * vi + av) * A.rec_stride) - ov;
+                            W[i] = __ldg(tr + (3 * vi + aw) * A.rec_stride) - ow;
+                        } else {
+                            U[i] = ts[(3 * vi + ax) * 32];
+                            V[i] = ts[(3 * vi + av) * 32] - ov;
+                            W[i] = ts[(3 * vi + aw) * 32] - ow;
+                        }
                     }
-                    f_w = ts[12 * 32];
+                    f_w = REC ? __ldg(tr + 12 * A.rec_stride) : ts[12 * 32];
                     if (slot6_dirty) { poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; slot6_dirty = false; }
                     const LBResult lb = tri_square_clip<32>(poly, U, V, W);
                     FaceClip fc;
@@ -959,7 +989,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS) k_deposit_tiles(Dep
                         if (local < n) break;
                         local -= n; ++f; sc >>= 8;
                     }
-                    unsigned long long rw = wrect[f * 32 + slot];
+                    unsigned long long rw = REC ? __ldg(A.rec_rows + f * A.rec_stride + rb + slot) : wrect[f * 32 + slot];
                     cv = (int)(rw & 7ull);
                     rw >>= 3;
 #pragma unroll

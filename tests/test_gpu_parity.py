@@ -352,11 +352,16 @@ def test_pair_record_buffer_modes_agree(psd, ctx, oracle, records):
     hg = torch.full((G, G, G), -1.0, dtype=torch.float64).pin_memory()
     ctx.psd_deposit_uniform_host(torch.from_numpy(pos).pin_memory(), G, hg)
     assert_parity(hg.numpy(), ora, what=f"records={records}, host output")
-    # a tiny grid where a tet's range meets a tile in several periodic images
+    # a tiny grid where a tet's range meets a tile in several periodic images (the records-only
+    # deposit kernel is not used there: the largest cell range plus a tile does not fit the grid)
     pos = crossing_field(12, 2.0)
-    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, 8)
-    ctx.psd_build_tets(to_dev(pos))
-    assert_parity(ctx.psd_deposit_uniform(8).cpu().numpy(), ora, what=f"records={records}, images")
+    for G in (8, 16, 24):
+        ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+        ctx.psd_build_tets(to_dev(pos))
+        assert_parity(ctx.psd_deposit_uniform(G).cpu().numpy(), ora, what=f"records={records}, images, G={G}")
+        s = ctx.psd_get_stats()
+        lo_hi = [oracle.build_tet(pos, 1.0, G, i, j, k, t)[2:] for i in range(12) for j in range(12) for k in range(12) for t in range(6)]
+        assert s.max_extent == max(int((hi - lo).max()) + 1 for lo, hi in lo_hi)
 
 
 def test_error_codes(psd, ctx):
