@@ -258,11 +258,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         }
         if (rec_cap) {
             char* rb = ctx->records.as<char>();
-            A.rec_stride = (long long)rec_cap;
             A.rec_g = reinterpret_cast<const double*>(rb);
-            A.rec_rows = reinterpret_cast<const unsigned long long*>(rb + 13 * 8 * rec_cap);
-            A.rec_word = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap);
-            A.rec_cnts = reinterpret_cast<const unsigned int*>(rb + 17 * 8 * rec_cap + 4 * rec_cap);
         }
         // The records-only deposit kernel needs every pair to meet its tile in one periodic image:
         // true when the largest cell range of a tet plus a tile fits the (coarsest) grid.

@@ -412,15 +412,27 @@ struct DepositArgs {
     int chord_axis;   // -1 adaptive, else 0..2
     unsigned long long* stats;
     double acc_scale, acc_inv_scale;  // fixed-point tile accumulators (PSD_ACC_FIXED): a power of two and its inverse
-    // pair records (k_pair_records -> k_deposit_tiles), structure of arrays with stride rec_stride;
+    // pair records (k_pair_records -> k_deposit_tiles), 18 doubles (144 bytes) each, one after the
+    // other (a pair's data sits in two cache lines: the jobs of a slot read it through L1):
+    //   [0..11] tile-local vertex coordinates (vertex v, axis x at 3 v + x), [12] weight (or the
+    //   value of a "special" add), [13..16] the four faces' row words (u64), [17] word | cnts << 32.
     // rec_g == nullptr: the deposit kernel runs stage A itself (fused mode)
-    const double* rec_g;              // [13][rec_stride]
-    const unsigned long long* rec_rows;  // [4][rec_stride]
-    const unsigned int* rec_word;     // [rec_stride]
-    const unsigned int* rec_cnts;     // [rec_stride]
-    long long rec_stride;
+    const double* rec_g;
     unsigned long long rec_pair_begin;  // first pair (position in pair_ids) of the record buffer
 };
+
+constexpr int REC_DOUBLES = 18;
+__device__ __forceinline__ double rec_d(const DepositArgs& A, long long r, int c) { return __ldg(A.rec_g + r * REC_DOUBLES + c); }
+__device__ __forceinline__ unsigned long long rec_rows(const DepositArgs& A, long long r, int f) {
+    return __ldg(reinterpret_cast<const unsigned long long*>(A.rec_g) + r * REC_DOUBLES + 13 + f);
+}
+__device__ __forceinline__ unsigned int rec_word(const DepositArgs& A, long long r) {
+    return __ldg(reinterpret_cast<const unsigned int*>(A.rec_g) + r * (2 * REC_DOUBLES) + 34);
+}
+__device__ __forceinline__ unsigned int rec_cnts(const DepositArgs& A, long long r) {
+    return __ldg(reinterpret_cast<const unsigned int*>(A.rec_g) + r * (2 * REC_DOUBLES) + 35);
+}
+
 
 
 // a6, the tile accumulator.  Shared memory has no native 64-bit atomic add on sm_100a (fp64 and
@@ -691,8 +703,7 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
 }
 
 // The pair records of a range of work items: stage A of every pair (image 0), one thread per pair,
-// written field by field (structure of arrays over the record index: the deposit kernel reads
-// them coalesced).  Splitting stage A off keeps the deposit kernel's instruction footprint inside
+// written record by record (18 doubles each; the deposit kernel's jobs read a slot's record through L1).  Splitting stage A off keeps the deposit kernel's instruction footprint inside
 // the 32 KB instruction cache (with stage A inlined 18 % of its stall samples were no-instruction).
 // Record index = (pair's position in the item, taken from the item's end) + item.begin - rec_pair_begin.
 constexpr int REC_THREADS = 128;
@@ -700,10 +711,13 @@ constexpr int REC_THREADS = 128;
 #define REC_MIN_CTAS 6
 #endif
 __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(DepositArgs A) {
-    __shared__ double swt[REC_THREADS / 32][13 * 32];
-    __shared__ unsigned long long swr[REC_THREADS / 32][4 * 32];
+    // per warp: the 32 records field by field, [18][32] 8-byte words (rows 0..12 doubles, 13..16 the
+    // row words, 17 word | cnts << 32), written out as one contiguous block of 32 x 18 words
+    __shared__ unsigned long long stg[REC_THREADS / 32][REC_DOUBLES * 32];
     __shared__ unsigned int sww[REC_THREADS / 32][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* swt = reinterpret_cast<double*>(stg[warp]);
+    unsigned long long* swr = stg[warp] + 13 * 32;
     const Item item = A.items[blockIdx.x];
     int level, org[3];
     double* out;
@@ -715,20 +729,28 @@ __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(Depo
         const unsigned int k = k0 + threadIdx.x;
         const bool have = k < item.count;
         const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - k)] : 0u;
-        const StageA sa = stage_a(A, have, id, 0, org, Gl, scale, &swt[warp][lane], &swr[warp][lane], &sww[warp][lane]);
+        __syncwarp();
+        const StageA sa = stage_a(A, have, id, 0, org, Gl, scale, swt + lane, swr + lane, &sww[warp][lane]);
         if (have) {
-            const long long r = (long long)(item.begin - A.rec_pair_begin) + k;
-            double* g = const_cast<double*>(A.rec_g);
+            if (sa.special) swt[12 * 32 + lane] = sa.special_val;
+            const unsigned int word = (sww[warp][lane] & 0xffu) | (unsigned int)sa.special << 8 |
+                                      (unsigned int)sa.special_cell << 9 | (unsigned int)min(sa.my_images, 16383) << 18;
+            stg[warp][17 * 32 + lane] = (unsigned long long)word | (unsigned long long)sa.cnts << 32;
+        }
+        __syncwarp();
+        // the warp's records (k0 + 32 warp .. + 31, those that exist) as one coalesced block
+        const unsigned int kw = k0 + 32u * warp;
+        if (kw < item.count) {
+            const int valid = (int)min(32u, item.count - kw);
+            unsigned long long* dst = reinterpret_cast<unsigned long long*>(const_cast<double*>(A.rec_g)) +
+                                      ((long long)(item.begin - A.rec_pair_begin) + kw) * REC_DOUBLES;
 #pragma unroll
-            for (int c = 0; c < 12; ++c) g[c * A.rec_stride + r] = swt[warp][c * 32 + lane];
-            g[12 * A.rec_stride + r] = sa.special ? sa.special_val : swt[warp][12 * 32 + lane];
-            unsigned long long* rw = const_cast<unsigned long long*>(A.rec_rows);
-#pragma unroll
-            for (int f = 0; f < 4; ++f) rw[f * A.rec_stride + r] = swr[warp][f * 32 + lane];
-            const_cast<unsigned int*>(A.rec_word)[r] = (sww[warp][lane] & 0xffu) | (unsigned int)sa.special << 8 |
-                                                        (unsigned int)sa.special_cell << 9 |
-                                                        (unsigned int)min(sa.my_images, 16383) << 18;
-            const_cast<unsigned int*>(A.rec_cnts)[r] = sa.cnts;
+            for (int q = 0; q < REC_DOUBLES; ++q) {
+                const int d = q * 32 + lane;
+                const int j = (d * 3641) >> 16;  // d / 18 for d < 576
+                const int c = d - j * REC_DOUBLES;
+                if (j < valid) dst[d] = stg[warp][c * 32 + j];
+            }
         }
     }
 }
@@ -801,23 +823,23 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
             if (REC) {
                 sa.cnts = 0u; sa.my_images = 1; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
                 if (have) {
-                    const unsigned int word = __ldg(A.rec_word + rb + lane);
-                    sa.cnts = __ldg(A.rec_cnts + rb + lane);
+                    const unsigned int word = rec_word(A, rb + lane);
+                    sa.cnts = rec_cnts(A, rb + lane);
                     sa.special = (word >> 8) & 1u;
                     sa.special_cell = (int)((word >> 9) & 511u);
-                    if (sa.special) sa.special_val = __ldg(A.rec_g + 12 * A.rec_stride + rb + lane);
+                    if (sa.special) sa.special_val = rec_d(A, rb + lane, 12);
                 }
             } else if (A.rec_g != nullptr && img == 0) {
                 sa.cnts = 0u; sa.my_images = 0; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
                 if (have) {
                     const long long r = (long long)(item.begin - A.rec_pair_begin) + (base + lane);
 #pragma unroll
-                    for (int c = 0; c < 13; ++c) wtet[c * 32 + lane] = A.rec_g[c * A.rec_stride + r];
+                    for (int c = 0; c < 13; ++c) wtet[c * 32 + lane] = rec_d(A, r, c);
 #pragma unroll
-                    for (int f = 0; f < 4; ++f) wrect[f * 32 + lane] = A.rec_rows[f * A.rec_stride + r];
-                    const unsigned int word = A.rec_word[r];
+                    for (int f = 0; f < 4; ++f) wrect[f * 32 + lane] = rec_rows(A, r, f);
+                    const unsigned int word = rec_word(A, r);
                     wword[lane] = word & 0xffu;
-                    sa.cnts = A.rec_cnts[r];
+                    sa.cnts = rec_cnts(A, r);
                     sa.special = (word >> 8) & 1u;
                     sa.special_cell = (int)((word >> 9) & 511u);
                     sa.special_val = wtet[12 * 32 + lane];
@@ -839,12 +861,12 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                 double f_w = 0.0;
                 if (act) {
                     if (COUNT) cnt.jobs++;
-                    const unsigned int word = REC ? __ldg(A.rec_word + rb + slot) : wword[slot];
+                    const unsigned int word = REC ? rec_word(A, rb + slot) : wword[slot];
                     const int ax = word & 3, c_lo = (word >> 2) & 7, c_hi = (word >> 5) & 7;
                     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
                     // the face triangle, column-local
                     const double* ts = wtet + slot;
-                    const double* tr = A.rec_g + rb + slot;   // REC: the slot's record, row c at tr[c * rec_stride]
+                    const long long rs = rb + slot;           // REC: the slot's record
                     const unsigned int fv = FACE_TABLE >> (6 * f);
                     const double ov = (double)cv, ow = (double)cw;
                     double U[3], V[3], W[3];
@@ -852,16 +874,16 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                     for (int i = 0; i < 3; ++i) {
                         const int vi = (fv >> (2 * i)) & 3;
                         if (REC) {
-                            U[i] = __ldg(tr + (3 * vi + ax) * A.rec_stride);
-                            V[i] = __ldg(tr + (3 * vi + av) * A.rec_stride) - ov;
-                            W[i] = __ldg(tr + (3 * vi + aw) * A.rec_stride) - ow;
+                            U[i] = rec_d(A, rs, 3 * vi + ax);
+                            V[i] = rec_d(A, rs, 3 * vi + av) - ov;
+                            W[i] = rec_d(A, rs, 3 * vi + aw) - ow;
                         } else {
                             U[i] = ts[(3 * vi + ax) * 32];
                             V[i] = ts[(3 * vi + av) * 32] - ov;
                             W[i] = ts[(3 * vi + aw) * 32] - ow;
                         }
                     }
-                    f_w = REC ? __ldg(tr + 12 * A.rec_stride) : ts[12 * 32];
+                    f_w = REC ? rec_d(A, rs, 12) : ts[12 * 32];
                     if (slot6_dirty) { poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; slot6_dirty = false; }
                     const LBResult lb = tri_square_clip<32>(poly, U, V, W);
                     FaceClip fc;
@@ -989,7 +1011,7 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                         if (local < n) break;
                         local -= n; ++f; sc >>= 8;
                     }
-                    unsigned long long rw = REC ? __ldg(A.rec_rows + f * A.rec_stride + rb + slot) : wrect[f * 32 + slot];
+                    unsigned long long rw = REC ? rec_rows(A, rb + slot, f) : wrect[f * 32 + slot];
                     cv = (int)(rw & 7ull);
                     rw >>= 3;
 #pragma unroll
