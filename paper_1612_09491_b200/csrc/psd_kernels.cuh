@@ -823,6 +823,8 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
             if (REC) {
                 sa.cnts = 0u; sa.my_images = 1; sa.special = false; sa.special_cell = 0; sa.special_val = 0.0;
                 if (have) {
+                    // the slot's record into L1 ahead of its jobs (its tail is read just below)
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(A.rec_g + (rb + lane) * REC_DOUBLES));
                     const unsigned int word = rec_word(A, rb + lane);
                     sa.cnts = rec_cnts(A, rb + lane);
                     sa.special = (word >> 8) & 1u;
