@@ -546,6 +546,7 @@ struct StageA {
     int special_cell;    // cell of the tile, (x*8+y)*8+z
     double special_val;
 };
+template <int SS>  // SS: stride of the [.][32] blocks in elements (32; 33 where they are read transposed)
 __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have, const unsigned int id, const int img,
                                           const int org[3], const int Gl, const double scale, double* wt,
                                           unsigned long long* wr, unsigned int* ww) {
@@ -579,10 +580,10 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
                         gl[v][x] = t.g[v][x] - (double)o;
-                        wt[(3 * v + x) * 32] = gl[v][x];
+                        wt[(3 * v + x) * SS] = gl[v][x];
                     }
                 }
-                wt[12 * 32] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
+                wt[12 * SS] = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
                 int ax = A.chord_axis;
                 if (ax < 0) {  // longest extent inside the tile -> fewest, longest columns
                     int e0 = hi[0] - lo[0], e1 = hi[1] - lo[1], e2 = hi[2] - lo[2];
@@ -619,8 +620,8 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
                     constexpr double ROW_EPS = 1e-9;
 #pragma unroll
                     for (int v = 0; v < 4; ++v) {
-                        const double pu = wt[(3 * v + ax) * 32], pv = wt[(3 * v + av) * 32];
-                        const double pw = wt[(3 * v + aw) * 32];
+                        const double pu = wt[(3 * v + ax) * SS], pv = wt[(3 * v + av) * SS];
+                        const double pw = wt[(3 * v + aw) * SS];
                         fv[v] = __double2int_rd(pv); cvv[v] = __double2int_ru(pv);
                         fw[v] = __double2int_rd(pw); cww[v] = __double2int_ru(pw);
                         cuu[v] = __double2int_ru(pu);
@@ -690,13 +691,13 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
                             }
                         }
                         o.cnts |= (unsigned int)c << (8 * f);
-                        wr[f * 32] = rows;
+                        wr[f * SS] = rows;
                     }
                     rect_written = true;
                 }
                 const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
                 const int hiu = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
-                if (!rect_written) { wr[0] = 0ull; wr[32] = 0ull; wr[64] = 0ull; wr[96] = 0ull; }
+                if (!rect_written) { wr[0] = 0ull; wr[SS] = 0ull; wr[2 * SS] = 0ull; wr[3 * SS] = 0ull; }
                 *ww = (unsigned int)(ax | lou << 2 | hiu << 5);
             }
     return o;
@@ -713,11 +714,12 @@ constexpr int REC_THREADS = 128;
 __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(DepositArgs A) {
     // per warp: the 32 records field by field, [18][32] 8-byte words (rows 0..12 doubles, 13..16 the
     // row words, 17 word | cnts << 32), written out as one contiguous block of 32 x 18 words
-    __shared__ unsigned long long stg[REC_THREADS / 32][REC_DOUBLES * 32];
+    constexpr int SS = 33;  // padded: the block is read transposed when it is written out
+    __shared__ unsigned long long stg[REC_THREADS / 32][REC_DOUBLES * SS];
     __shared__ unsigned int sww[REC_THREADS / 32][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     double* swt = reinterpret_cast<double*>(stg[warp]);
-    unsigned long long* swr = stg[warp] + 13 * 32;
+    unsigned long long* swr = stg[warp] + 13 * SS;
     const Item item = A.items[blockIdx.x];
     int level, org[3];
     double* out;
@@ -730,12 +732,12 @@ __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(Depo
         const bool have = k < item.count;
         const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - k)] : 0u;
         __syncwarp();
-        const StageA sa = stage_a(A, have, id, 0, org, Gl, scale, swt + lane, swr + lane, &sww[warp][lane]);
+        const StageA sa = stage_a<SS>(A, have, id, 0, org, Gl, scale, swt + lane, swr + lane, &sww[warp][lane]);
         if (have) {
-            if (sa.special) swt[12 * 32 + lane] = sa.special_val;
+            if (sa.special) swt[12 * SS + lane] = sa.special_val;
             const unsigned int word = (sww[warp][lane] & 0xffu) | (unsigned int)sa.special << 8 |
                                       (unsigned int)sa.special_cell << 9 | (unsigned int)min(sa.my_images, 16383) << 18;
-            stg[warp][17 * 32 + lane] = (unsigned long long)word | (unsigned long long)sa.cnts << 32;
+            stg[warp][17 * SS + lane] = (unsigned long long)word | (unsigned long long)sa.cnts << 32;
         }
         __syncwarp();
         // the warp's records (k0 + 32 warp .. + 31, those that exist) as one coalesced block
@@ -749,7 +751,7 @@ __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(Depo
                 const int d = q * 32 + lane;
                 const int j = (d * 3641) >> 16;  // d / 18 for d < 576
                 const int c = d - j * REC_DOUBLES;
-                if (j < valid) dst[d] = stg[warp][c * 32 + j];
+                if (j < valid) dst[d] = stg[warp][c * SS + j];
             }
         }
     }
@@ -848,7 +850,7 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                     sa.my_images = (int)(word >> 18);
                 }
             } else {
-                sa = stage_a(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
+                sa = stage_a<32>(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
             }
             if (sa.special) tile_add(acc + sa.special_cell, tile_share(sa.special_val, A.acc_scale));
             const unsigned int cnts = sa.cnts;
