@@ -466,21 +466,23 @@ __device__ __forceinline__ TileShare tile_share(double x, double scale) {
 #endif
     return q;
 }
-__device__ __forceinline__ void tile_add(double* cell, TileShare q) {
+// The two limbs of cell i are at words i and 512 + i of the tile (not next to each other: the
+// cells of the lanes of a warp then spread over all 32 banks).
+__device__ __forceinline__ void tile_add(double* acc, int i, TileShare q) {
 #if PSD_ACC_FIXED
-    unsigned int* a = reinterpret_cast<unsigned int*>(cell);
+    unsigned int* a = reinterpret_cast<unsigned int*>(acc) + i;
     const unsigned int old = atomicAdd(a, q.lo);
-    atomicAdd(a + 1, q.hi + (unsigned int)(old + q.lo < old));
+    atomicAdd(a + TILE_CELLS, q.hi + (unsigned int)(old + q.lo < old));
 #else
-    atomicAdd(cell, q.x);
+    atomicAdd(acc + i, q.x);
 #endif
 }
-__device__ __forceinline__ double tile_value(const double* cell, double inv_scale) {
+__device__ __forceinline__ double tile_value(const double* acc, int i, double inv_scale) {
 #if PSD_ACC_FIXED
-    const unsigned int* a = reinterpret_cast<const unsigned int*>(cell);
-    return (double)(long long)(((unsigned long long)a[1] << 32) | a[0]) * inv_scale;
+    const unsigned int* a = reinterpret_cast<const unsigned int*>(acc);
+    return (double)(long long)(((unsigned long long)a[TILE_CELLS + i] << 32) | a[i]) * inv_scale;
 #else
-    return *cell;
+    return acc[i];
 #endif
 }
 
@@ -852,7 +854,7 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
             } else {
                 sa = stage_a<32>(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
             }
-            if (sa.special) tile_add(acc + sa.special_cell, tile_share(sa.special_val, A.acc_scale));
+            if (sa.special) tile_add(acc, sa.special_cell, tile_share(sa.special_val, A.acc_scale));
             const unsigned int cnts = sa.cnts;
             if (!REC && img == 0) max_images = __reduce_max_sync(0xffffffffu, sa.my_images);
             // ---- stages B + C for 32 jobs (a lambda with a single call site: its code is large).
@@ -920,14 +922,14 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                                 for (int cc = 0; cc < TILE; ++cc) {
                                     const int c = c_lo + cc;
                                     if (c > full_hi) break;
-                                    tile_add(acc + colofs + c * su, qA);
+                                    tile_add(acc, colofs + c * su, qA);
                                     if (COUNT) cnt.cells++;
                                 }
                             }
                             if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {  // the cell holding umin
                                 const double D = fma(-(double)fc.ifl, fc.A, fc.M1);
                                 if (D != 0.0) {
-                                    tile_add(acc + colofs + fc.ifl * su, tile_share(f_w * D, A.acc_scale));
+                                    tile_add(acc, colofs + fc.ifl * su, tile_share(f_w * D, A.acc_scale));
                                     if (COUNT) cnt.cells++;
                                 }
                             }
@@ -972,8 +974,8 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                                          (1.0 / 6.0) * s_w;
                         if (COUNT) cnt.plane_evals++;
                         if (R != 0.0) {
-                            if (a <= c_hi) { tile_add(acc + colofs + a * su, tile_share(R, A.acc_scale)); if (COUNT) cnt.cells++; }
-                            if (a - 1 >= c_lo) { tile_add(acc + colofs + (a - 1) * su, tile_share(-R, A.acc_scale)); if (COUNT) cnt.cells++; }
+                            if (a <= c_hi) { tile_add(acc, colofs + a * su, tile_share(R, A.acc_scale)); if (COUNT) cnt.cells++; }
+                            if (a - 1 >= c_lo) { tile_add(acc, colofs + (a - 1) * su, tile_share(-R, A.acc_scale)); if (COUNT) cnt.cells++; }
                         }
                     }
                 }
@@ -1033,7 +1035,7 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
     __syncthreads();
     // ---- a6: flush the tile with fp64 reductions (other work items may hold the same tile)
     for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) {
-        const double v = tile_value(acc + i, A.acc_inv_scale);
+        const double v = tile_value(acc, i, A.acc_inv_scale);
         if (v != 0.0) {
             int cz = i & 7, cy = (i >> 3) & 7, cx = i >> 6;
             atomicAdd(out + cx * str[0] + cy * str[1] + cz, v);
