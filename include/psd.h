@@ -87,6 +87,12 @@ enum {
                                 buffer holds up to 48 Mi pairs and is refilled slab by slab.
                                 0: the deposit kernel runs stage A itself (no record buffer).
                                 A value > 1 sets the buffer's capacity in pairs (tests).       */
+    PSD_OPT_ROWS_FP32 = 9,     /* binned path with pair records, a4: which columns of a row of a face's
+                                rectangle the face meets (the face jobs) is decided in fp32 with a
+                                margin that covers fp32's rounding (1, default) or in fp64 with a
+                                margin of 1e-9 (0).  Either set holds every column with a non-empty
+                                polygon and the clip itself is fp64, so the deposit is the same;
+                                fp32 admits a few more empty jobs (n_face_jobs).               */
     PSD_OPT_PATCH_RESTRICT = 7  /* psd_deposit_patches, PAPER.md:193 (coarser representations of the
                                 internal nodes).  1 (default): a listed patch whose 8 children are
                                 all listed too is not deposited into; it is filled afterwards by
@@ -132,6 +138,8 @@ typedef struct {
     int64_t n_restricted_patches; /* psd_deposit_patches: patches filled from their children     */
     int64_t n_general_clips; /* counters: face jobs the straight-line clip passed to the general
                                convex clip (a tie within its margin: lattice-aligned input)  */
+    int64_t n_rows_missed;   /* counters, PSD_OPT_ROWS_FP32 = 1: rows of faces whose fp64 column range
+                               the fp32 classification does not cover (a self-check: 0)       */
     /* device pointer to the per-(tile, size class) pair counts of the last binned deposit
        (2 * n_tiles uint32, see psd_get_tile_class_counts) */
     const uint32_t* tile_counts_dev;

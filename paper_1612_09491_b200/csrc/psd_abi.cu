@@ -47,7 +47,7 @@ struct psd_ctx {
     bool built = false;
     double total_mass = 0.0;
     int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1,
-        use_records = 1;
+        use_records = 1, rows_fp32 = 1;
     unsigned long long rec_pairs_max = 48ull << 20;  // capacity of the pair-record buffer (REC_PAIRS_MAX)
     long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 2048;
@@ -272,7 +272,9 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                 A.items = items0 + bounds[i].item;
                 A.rec_pair_begin = bounds[i].pair;
                 if (rec_cap) {
-                    k_pair_records<<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
+                    if (ctx->rows_fp32 && ctx->counters) k_pair_records<2><<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
+                    else if (ctx->rows_fp32) k_pair_records<1><<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
+                    else k_pair_records<0><<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
                     ctx->launches += 1;
                 }
                 if (rec_only) {
@@ -769,6 +771,7 @@ int psd_get_stats(psd_ctx* ctx, psd_stats* out) {
         s.n_plane_evals = (int64_t)ctx->pinned[ST_PLANE_CLIPS];
         s.n_cells_written = (int64_t)ctx->pinned[ST_CELLS];
         s.n_general_clips = (int64_t)ctx->pinned[ST_GENERAL];
+        s.n_rows_missed = (int64_t)ctx->pinned[ST_ROWS_MISSED];
         for (int i = 0; i < 64; ++i) {
             s.hist_tet[i] = ctx->pinned[ST_COUNT + i];
             s.hist_pair[i] = ctx->pinned[ST_COUNT + 64 + i];
@@ -845,6 +848,9 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
             ctx->use_records = value != 0.0;
             ctx->rec_pairs_max = value > 1.0 ? (unsigned long long)value : REC_PAIRS_MAX;
             return PSD_OK;
+        case PSD_OPT_ROWS_FP32:
+            if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "fp32 rows must be 0 or 1");
+            ctx->rows_fp32 = iv; return PSD_OK;
         case PSD_OPT_PATCH_RESTRICT:
             if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "patch restriction must be 0 or 1");
             ctx->patch_restrict = iv; return PSD_OK;

@@ -49,7 +49,7 @@ constexpr int N_CLASSES = 2;
 constexpr long long CLASS_SMALL_MAX_CELLS = 8;  // default of PSD_OPT_CLASS_SMALL_CELLS
 
 enum { ST_SUM_CELLS = 0, ST_MAX_CELLS, ST_INVERTED, ST_DEGENERATE, ST_UNWRAP, ST_NONFINITE,
-       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_GENERAL, ST_MAX_EXTENT, ST_COUNT };
+       ST_PAIRS, ST_TASKS, ST_FACE_CLIPS, ST_PLANE_CLIPS, ST_CELLS, ST_GENERAL, ST_MAX_EXTENT, ST_ROWS_MISSED, ST_COUNT };
 
 // ---------------------------------------------------------------- validation of positions
 __global__ void k_validate(Particles p, unsigned long long* stats) {
@@ -541,19 +541,182 @@ __device__ __forceinline__ void tile_geometry(const Space& s, unsigned int tile,
 //   wr [4][32]  u64      per face: first row (3 bits), then 7 bits per row: first column, columns
 //   ww [32]     u32      chord axis (2 bits), first / last cell of the tet along it in the tile
 // A tet that goes to one cell whole (inside one cell, or degenerate) is returned as a "special" add.
+//
+// a4 in this formulation is the classification of (face, column) jobs: which columns of a row of
+// the face's rectangle the triangle really meets (face_rows).  It runs in fp64 with a 1e-9 margin,
+// or in fp32 with a margin that covers fp32's rounding ("fp32 classification
+// with a conservative margin, fp64 clip for the survivors"): either way the set of jobs contains
+// every column with a non-empty polygon, a job too many clips to nothing, so the deposit is the same.
+template <typename T> struct RowNum;
+template <> struct RowNum<double> {
+    static constexpr bool exact_rect = true;
+    static __device__ __forceinline__ int fl(double x) { return __double2int_rd(x); }
+    static __device__ __forceinline__ int ce(double x) { return __double2int_ru(x); }
+    static __device__ __forceinline__ double rcp(double x) { return fast_rcp(x); }
+    static __device__ __forceinline__ double mad(double a, double b, double c) { return fma(a, b, c); }
+};
+template <> struct RowNum<float> {
+    static constexpr bool exact_rect = false;
+    static __device__ __forceinline__ int fl(float x) { return __float2int_rd(x); }
+    static __device__ __forceinline__ int ce(float x) { return __float2int_ru(x); }
+    static __device__ __forceinline__ float rcp(float x) {
+        float r;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float mad(float a, float b, float c) { return fmaf(a, b, c); }
+};
+
+// The row words of a tet's four faces (first row in bits 0..2, then 7 bits per row: first column
+// (3), columns (4)) and the faces' job counts (8 bits each).  pu/pv/pw: the 4 vertices, tile-local;
+// [lov,hiv] x [low,hiw]: the tet's cell range in the tile across the chord axis, lou: its first
+// cell along it.  The w-extremes of (triangle n row strip) are at vertices inside the strip or
+// where an edge crosses one of the strip's two lines.
+//   T = double: rectangles exact, rows / columns with a margin of 1e-9 (a point that close to a
+//       lattice line counts for both sides).
+//   T = float:  with a = max |coordinate|, every rounded coordinate and difference is within
+//       2^-23 a of its value, so e0 = 2^-19 a covers the row a vertex is in; a crossing point
+//       w = w_i - (v_i - L) dw/dv is within 2^-23 a (3 |dw/dv| + 5) of its value when |dv| > e0 / 2
+//       (then dv is known to 25 %), and when |dv| <= e0 / 2 both ends of the edge are within e0 of
+//       the line, count for both rows, and the crossing lies between them; a crossing that the
+//       rounded signs miss is within |dw/dv| 2^-23 a of a vertex that counts for both rows.  So
+//       em = e0 (1 + max |dw/dv| over the tet's edges) covers every column decision.
+template <typename T>
+__device__ __forceinline__ unsigned int face_rows(const double pu[4], const double pv[4], const double pw[4],
+                                                  const int lov, const int hiv, const int low, const int hiw,
+                                                  const int lou, unsigned long long rows4[4]) {
+    using R = RowNum<T>;
+    T pvv[4], pww[4];
+    T e0, em, er, erw;  // margins: row of a vertex, column of a point, rectangle rows, rectangle columns
+    T slope[6];         // dw/dv of the 6 edges (i < j), index i + j - (i == 0 ? 1 : 0): 01 02 03 12 13 23
+#pragma unroll
+    for (int v = 0; v < 4; ++v) { pvv[v] = (T)pv[v]; pww[v] = (T)pw[v]; }
+    T smax = (T)0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = i + 1; j < 4; ++j) {
+            const T dvv = pvv[j] - pvv[i];
+            const T sl = (pww[j] - pww[i]) * R::rcp(dvv == (T)0 ? (T)1 : dvv);
+            slope[i + j - (i == 0 ? 1 : 0)] = sl;
+            if (!R::exact_rect) smax = fmax(smax, fabs(sl));
+        }
+    T puu[4];
+    if (R::exact_rect) {
+        e0 = (T)1e-9; em = (T)1e-9; er = (T)0; erw = (T)0;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) puu[v] = (T)pu[v];
+    } else {
+        T amax = (T)1;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            puu[v] = (T)pu[v];
+            amax = fmax(amax, fmax(fabs(puu[v]), fmax(fabs(pvv[v]), fabs(pww[v]))));
+        }
+        e0 = amax * (T)0x1p-19;
+        em = R::mad(e0, smax, e0);
+        er = e0; erw = em;
+    }
+    // per vertex: floor / ceil of (v, w) and ceil of u for the faces' rectangles (integer min / max:
+    // floor and ceil are monotone); rows / columns the vertex belongs to with the margin
+    int fv[4], cvv[4], fw[4], cww[4], cuu[4], rlo[4], rhi[4], klo[4], khi[4];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        rlo[v] = R::fl(pvv[v] - e0); rhi[v] = R::fl(pvv[v] + e0);
+        klo[v] = R::fl(pww[v] - em); khi[v] = R::fl(pww[v] + em);
+        if (R::exact_rect) {
+            fv[v] = R::fl(pvv[v]); fw[v] = R::fl(pww[v]);
+        } else {
+            fv[v] = rlo[v]; fw[v] = klo[v];
+        }
+        cvv[v] = R::ce(pvv[v] + er); cww[v] = R::ce(pww[v] + erw);
+        cuu[v] = R::ce(puu[v] + er);
+    }
+    // columns met by the face's three edges on the lattice line v = L (with the margin)
+    auto line_cols = [&](const int a, const int b, const int d, const int L, int& clo, int& chi) {
+        clo = 99; chi = -99;
+        const int e0i[3] = {a, b, a}, e1i[3] = {b, d, d};   // edges with i < j: (a,b) (b,d) (a,d)
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const int i = e0i[e], j = e1i[e];
+            const T di = pvv[i] - (T)L, dj = pvv[j] - (T)L;
+            if (di * dj < (T)0) {
+                const T w = R::mad(-di, slope[i + j - (i == 0 ? 1 : 0)], pww[i]);
+                clo = min(clo, R::fl(w - em));
+                chi = max(chi, R::fl(w + em));
+            }
+        }
+    };
+    unsigned int cnts = 0u;
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
+        const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;   // a < b < d
+        // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
+        const int v0 = max(min(min(fv[a], fv[b]), fv[d]), lov);
+        const int v1 = min(max(max(cvv[a], cvv[b]), cvv[d]) - 1, hiv);
+        const int w0 = max(min(min(fw[a], fw[b]), fw[d]), low);
+        const int w1 = min(max(max(cww[a], cww[b]), cww[d]) - 1, hiw);
+        int c = 0;
+        unsigned long long rows = 0ull;
+        if (v1 >= v0 && w1 >= w0 && max(max(cuu[a], cuu[b]), cuu[d]) > lou) {
+            rows = (unsigned long long)v0;
+            int llo, lhi;
+            line_cols(a, b, d, v0, llo, lhi);
+#pragma unroll 1
+            for (int r = v0; r <= v1; ++r) {
+                int ulo, uhi;
+                line_cols(a, b, d, r + 1, ulo, uhi);
+                int rl = min(llo, ulo), rh = max(lhi, uhi);
+                if (rlo[a] <= r && r <= rhi[a]) { rl = min(rl, klo[a]); rh = max(rh, khi[a]); }
+                if (rlo[b] <= r && r <= rhi[b]) { rl = min(rl, klo[b]); rh = max(rh, khi[b]); }
+                if (rlo[d] <= r && r <= rhi[d]) { rl = min(rl, klo[d]); rh = max(rh, khi[d]); }
+                const int c0 = max(rl, w0), c1 = min(rh, w1);
+                const int n = max(c1 - c0 + 1, 0);
+                rows |= (unsigned long long)(n ? (c0 | n << 3) : 0) << (3 + 7 * (r - v0));
+                c += n;
+                llo = ulo; lhi = uhi;
+            }
+        }
+        cnts |= (unsigned int)c << (8 * f);
+        rows4[f] = rows;
+    }
+    return cnts;
+}
+
+// Rows of the fp64 classification that the other one does not cover (a check: must be 0).  Both
+// words: first row in bits 0..2, then 7 bits per row (first column, columns).
+__device__ __forceinline__ unsigned int rows_missed(const unsigned long long wide, const unsigned long long ref) {
+    const int v0w = (int)(wide & 7ull), v0r = (int)(ref & 7ull);
+    unsigned int missed = 0;
+#pragma unroll 1
+    for (int i = 0; i < TILE; ++i) {
+        const unsigned int fr = (unsigned int)(ref >> (3 + 7 * i)) & 127u;
+        const int n = (int)(fr >> 3);
+        if (n == 0) continue;
+        const int c0 = (int)(fr & 7u), k = v0r + i - v0w;
+        const unsigned int fw = (k >= 0 && k < TILE) ? (unsigned int)(wide >> (3 + 7 * k)) & 127u : 0u;
+        const int c0w = (int)(fw & 7u), nw = (int)(fw >> 3);
+        missed += !(nw > 0 && c0w <= c0 && c0w + nw >= c0 + n);
+    }
+    return missed;
+}
+
 struct StageA {
+    unsigned int missed; // ROWS = 2: rows of the fp64 classification not covered by the fp32 one
     unsigned int cnts;   // face jobs, 8 bits per face
     int my_images;       // periodic images of the tile this tet's range meets
     bool special;
     int special_cell;    // cell of the tile, (x*8+y)*8+z
     double special_val;
 };
-template <int SS>  // SS: stride of the [.][32] blocks in elements (32; 33 where they are read transposed)
+template <int SS, int ROWS>  // SS: stride of the [.][32] blocks in elements (32; 33 where they are read
+                             // transposed); ROWS: 0 the rows in fp64, 1 in fp32, 2 in fp32 and checked
+                             // against fp64 (face_rows)
 __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have, const unsigned int id, const int img,
                                           const int org[3], const int Gl, const double scale, double* wt,
                                           unsigned long long* wr, unsigned int* ww) {
     StageA o;
-    o.cnts = 0u; o.my_images = 0; o.special = false; o.special_cell = 0; o.special_val = 0.0;
+    o.cnts = 0u; o.my_images = 0; o.special = false; o.special_cell = 0; o.special_val = 0.0; o.missed = 0u;
             Tet t;
             double det = 1.0;
             int nimg[3] = {1, 1, 1}, mlo[3] = {0, 0, 0};
@@ -611,90 +774,29 @@ __device__ __forceinline__ StageA stage_a(const DepositArgs& A, const bool have,
                     o.special = true; o.special_cell = (lo[0] * TILE + lo[1]) * TILE + lo[2];
                     o.special_val = A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0);
                 } else {
-                    // per vertex: floor / ceil of (v, w) and ceil of u, read back through the
-                    // runtime axis (the lane's own stores above); the faces' rectangles are then
-                    // integer min / max (floor and ceil are monotone)
-                    int fv[4], cvv[4], fw[4], cww[4], cuu[4];
-                    // the same with a margin (a point within ROW_EPS of a lattice line counts for both
-                    // sides): rows / columns a vertex belongs to, for the per-row column ranges
-                    int rlo[4], rhi[4], klo[4], khi[4];
-                    double pvv[4], pww[4];
-                    constexpr double ROW_EPS = 1e-9;
+                    // per face the columns each row of its rectangle meets (row words + job counts),
+                    // in fp64 with a 1e-9 margin, or (F32) in fp32 with a margin that covers its rounding
+                    double pu4[4], pv4[4], pw4[4];
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) {
-                        const double pu = wt[(3 * v + ax) * SS], pv = wt[(3 * v + av) * SS];
-                        const double pw = wt[(3 * v + aw) * SS];
-                        fv[v] = __double2int_rd(pv); cvv[v] = __double2int_ru(pv);
-                        fw[v] = __double2int_rd(pw); cww[v] = __double2int_ru(pw);
-                        cuu[v] = __double2int_ru(pu);
-                        rlo[v] = __double2int_rd(pv - ROW_EPS); rhi[v] = __double2int_rd(pv + ROW_EPS);
-                        klo[v] = __double2int_rd(pw - ROW_EPS); khi[v] = __double2int_rd(pw + ROW_EPS);
-                        pvv[v] = pv; pww[v] = pw;
+                    for (int v = 0; v < 4; ++v) {  // read back through the runtime axis (the lane's own stores above)
+                        pu4[v] = wt[(3 * v + ax) * SS]; pv4[v] = wt[(3 * v + av) * SS]; pw4[v] = wt[(3 * v + aw) * SS];
                     }
                     const int lov = av == 0 ? lo[0] : (av == 1 ? lo[1] : lo[2]);
                     const int hiv = av == 0 ? hi[0] : (av == 1 ? hi[1] : hi[2]);
                     const int low = aw == 0 ? lo[0] : (aw == 1 ? lo[1] : lo[2]);
                     const int hiw = aw == 0 ? hi[0] : (aw == 1 ? hi[1] : hi[2]);
                     const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
-                    // dw/dv of the 6 edges (i < j), index i + j - (i == 0 ? 1 : 0): 01 02 03 12 13 23
-                    double slope[6];
+                    unsigned long long rows4[4];
+                    if (ROWS) o.cnts = face_rows<float>(pu4, pv4, pw4, lov, hiv, low, hiw, lou, rows4);
+                    else o.cnts = face_rows<double>(pu4, pv4, pw4, lov, hiv, low, hiw, lou, rows4);
+                    if (ROWS == 2) {
+                        unsigned long long ref4[4];
+                        face_rows<double>(pu4, pv4, pw4, lov, hiv, low, hiw, lou, ref4);
 #pragma unroll
-                    for (int i = 0; i < 3; ++i)
-#pragma unroll
-                        for (int j = i + 1; j < 4; ++j) {
-                            const double dvv = pvv[j] - pvv[i];
-                            slope[i + j - (i == 0 ? 1 : 0)] = (pww[j] - pww[i]) * fast_rcp(dvv == 0.0 ? 1.0 : dvv);
-                        }
-                    // columns met by the face's three edges on the lattice line v = L (with the margin)
-                    auto line_cols = [&](const int a, const int b, const int d, const int L, int& clo, int& chi) {
-                        clo = 99; chi = -99;
-                        const int e0[3] = {a, b, a}, e1[3] = {b, d, d};   // edges with i < j: (a,b) (b,d) (a,d)
-#pragma unroll
-                        for (int e = 0; e < 3; ++e) {
-                            const int i = e0[e], j = e1[e];
-                            const double di = pvv[i] - (double)L, dj = pvv[j] - (double)L;
-                            if (di * dj < 0.0) {
-                                const double w = fma(-di, slope[i + j - (i == 0 ? 1 : 0)], pww[i]);
-                                clo = min(clo, __double2int_rd(w - ROW_EPS));
-                                chi = max(chi, __double2int_rd(w + ROW_EPS));
-                            }
-                        }
-                    };
-#pragma unroll
-                    for (int f = 0; f < 4; ++f) {  // face f = the 3 vertices other than f
-                        const int a = f == 0 ? 1 : 0, b = f <= 1 ? 2 : 1, d = f == 3 ? 2 : 3;   // a < b < d
-                        // columns cv with minv < cv+1 and maxv > cv, inside the tet's tile range
-                        const int v0 = max(min(min(fv[a], fv[b]), fv[d]), lov);
-                        const int v1 = min(max(max(cvv[a], cvv[b]), cvv[d]) - 1, hiv);
-                        const int w0 = max(min(min(fw[a], fw[b]), fw[d]), low);
-                        const int w1 = min(max(max(cww[a], cww[b]), cww[d]) - 1, hiw);
-                        int c = 0;
-                        unsigned long long rows = 0ull;
-                        if (v1 >= v0 && w1 >= w0 && max(max(cuu[a], cuu[b]), cuu[d]) > lou) {
-                            // per row of the rectangle, the columns the triangle really meets: the
-                            // w-extremes of (triangle n row strip) are at vertices inside the strip or
-                            // where an edge crosses one of the strip's two lines -- no empty jobs
-                            rows = (unsigned long long)v0;
-                            int llo, lhi;
-                            line_cols(a, b, d, v0, llo, lhi);
-#pragma unroll 1
-                            for (int r = v0; r <= v1; ++r) {
-                                int ulo, uhi;
-                                line_cols(a, b, d, r + 1, ulo, uhi);
-                                int rl = min(llo, ulo), rh = max(lhi, uhi);
-                                if (rlo[a] <= r && r <= rhi[a]) { rl = min(rl, klo[a]); rh = max(rh, khi[a]); }
-                                if (rlo[b] <= r && r <= rhi[b]) { rl = min(rl, klo[b]); rh = max(rh, khi[b]); }
-                                if (rlo[d] <= r && r <= rhi[d]) { rl = min(rl, klo[d]); rh = max(rh, khi[d]); }
-                                const int c0 = max(rl, w0), c1 = min(rh, w1);
-                                const int n = max(c1 - c0 + 1, 0);
-                                rows |= (unsigned long long)(n ? (c0 | n << 3) : 0) << (3 + 7 * (r - v0));
-                                c += n;
-                                llo = ulo; lhi = uhi;
-                            }
-                        }
-                        o.cnts |= (unsigned int)c << (8 * f);
-                        wr[f * SS] = rows;
+                        for (int f = 0; f < 4; ++f) o.missed += rows_missed(rows4[f], ref4[f]);
                     }
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) wr[f * SS] = rows4[f];
                     rect_written = true;
                 }
                 const int lou = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]);
@@ -713,6 +815,7 @@ constexpr int REC_THREADS = 128;
 #ifndef REC_MIN_CTAS
 #define REC_MIN_CTAS 6
 #endif
+template <int ROWS>
 __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(DepositArgs A) {
     // per warp: the 32 records field by field, [18][32] 8-byte words (rows 0..12 doubles, 13..16 the
     // row words, 17 word | cnts << 32), written out as one contiguous block of 32 x 18 words
@@ -734,7 +837,8 @@ __global__ void __launch_bounds__(REC_THREADS, REC_MIN_CTAS) k_pair_records(Depo
         const bool have = k < item.count;
         const unsigned int id = have ? A.pair_ids[item.begin + (item.count - 1u - k)] : 0u;
         __syncwarp();
-        const StageA sa = stage_a<SS>(A, have, id, 0, org, Gl, scale, swt + lane, swr + lane, &sww[warp][lane]);
+        const StageA sa = stage_a<SS, ROWS>(A, have, id, 0, org, Gl, scale, swt + lane, swr + lane, &sww[warp][lane]);
+        if (ROWS == 2 && sa.missed) atomicAdd(&A.stats[ST_ROWS_MISSED], (unsigned long long)sa.missed);
         if (have) {
             if (sa.special) swt[12 * SS + lane] = sa.special_val;
             const unsigned int word = (sww[warp][lane] & 0xffu) | (unsigned int)sa.special << 8 |
@@ -852,7 +956,7 @@ __global__ void __launch_bounds__(DEP_THREADS, REC ? DEP_MIN_CTAS_REC : DEP_MIN_
                     sa.my_images = (int)(word >> 18);
                 }
             } else {
-                sa = stage_a<32>(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
+                sa = stage_a<32, 0>(A, have, id, img, org, Gl, scale, wtet + lane, wrect + lane, wword + lane);
             }
             if (sa.special) tile_add(acc, sa.special_cell, tile_share(sa.special_val, A.acc_scale));
             const unsigned int cnts = sa.cnts;

@@ -364,6 +364,40 @@ def test_pair_record_buffer_modes_agree(psd, ctx, oracle, records):
         assert s.max_extent == max(int((hi - lo).max()) + 1 for lo, hi in lo_hi)
 
 
+@pytest.mark.parametrize("case", ["crossing", "crossing_far", "lattice", "jittered", "tiny_cells"])
+def test_fp32_rows_cover_the_fp64_rows(psd, ctx, oracle, case):
+    """PSD_OPT_ROWS_FP32: which columns a face meets is decided in fp32 with a
+    margin, the clip stays fp64.  The fp32 set of jobs must hold every row range of the fp64 one
+    (n_rows_missed, checked on the device pair by pair), may hold a few more jobs, and the deposit
+    is the same."""
+    if case == "crossing":
+        pos, G = crossing_field(24, 1.5, dtype="float32", stride=4), 192
+    elif case == "crossing_far":   # long thin tets: coordinates far from the tile, steep edges
+        pos, G = crossing_field(16, 6.0), 256
+    elif case == "lattice":        # every vertex on a lattice line, every edge along one or through corners
+        pos, G = psd_inputs.lattice(16), 64
+    elif case == "jittered":
+        pos, G = psd_inputs.jittered_lattice(32, seed=5), 16
+    else:                          # tets far smaller than a cell: slopes of every size inside one column
+        pos, G = crossing_field(16, 0.5), 64
+    ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_set_option(psd.OPT_COUNTERS, 1)
+    ctx.psd_set_option(psd.OPT_CHUNK, 256)
+    res = {}
+    for mode in (0, 1):
+        ctx.psd_set_option(psd.OPT_ROWS_FP32, mode)
+        ctx.psd_build_tets(to_dev(pos))
+        g = ctx.psd_deposit_uniform(G)
+        s = ctx.psd_get_stats()
+        assert_parity(g.cpu().numpy(), ora, what=f"{case}, rows_fp32={mode}")
+        res[mode] = (g.cpu().numpy(), s.n_face_jobs, s.n_face_clips, s.n_rows_missed)
+    assert res[1][3] == 0 and res[0][3] == 0
+    # a few more jobs in fp32; on the exact lattice every vertex sits on lattice lines and the margin
+    # puts it on both sides of each (about twice the jobs, all but the fp64 ones empty)
+    assert res[0][1] <= res[1][1] <= (3.0 if case == "lattice" else 1.02) * res[0][1] + 64, (res[0][1], res[1][1])
+    assert np.abs(res[1][0] - res[0][0]).max() <= 1e-13 * max(1.0, np.abs(res[0][0]).max())
+
+
 def test_error_codes(psd, ctx):
     import torch
     with pytest.raises(psd.PsdError) as e:
