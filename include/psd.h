@@ -242,6 +242,40 @@ PSD_API const char* psd_last_error(const psd_ctx* ctx);
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 PSD_API int64_t psd_launch_count(const psd_ctx* ctx);
 
+/* ---- A deposit that allocates nothing ---------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture set-up, tight serving
+ * loops, harnesses that forbid allocation).  The same operation as psd_build_tets +
+ * psd_deposit_uniform on the binned path (census, counting sort by 8^3 tile,
+ * tile deposit with stage A inside the deposit kernel, i.e. PSD_OPT_PAIR_RECORDS = 0), default
+ * options, no context: all scratch (pair counts, offsets, work items, pair list) lives in ONE
+ * file-scope `static __device__` array of PSD_STATIC_SCRATCH_BYTES (about 16.3 MiB) that every
+ * GPU which loads the library holds until the process exits.  The call makes no cudaMalloc,
+ * cudaFree, cudaMallocHost, event or stream creation, and calls no allocating library routine.
+ *
+ *   device, cuda_stream   the device is made current; all work is enqueued on the stream
+ *   pos_dev      device, borrowed: N^3 particles as for psd_build_tets (dtype, stride_elems)
+ *   N            2 .. PSD_STATIC_MAX_N
+ *   G            a multiple of 8 in 8 .. PSD_STATIC_MAX_G
+ *   grid_dev     device, caller-owned, double[G^3], index (ix*G+iy)*G+iz; overwritten
+ *   n_pairs_out  host, may be NULL: number of (tet, tile) pairs of this deposit
+ *   err, err_len host, may be NULL / 0: receives a message when the return value is not PSD_OK
+ *
+ * Limits (else PSD_ERR_INVALID_ARG with a message naming the limit, nothing deposited): N, G as
+ * above, and at most PSD_STATIC_MAX_PAIRS (tet, tile) pairs (known only after the census: the
+ * grid is then left zero-filled).  Positions with NaN/Inf are rejected like psd_build_tets.
+ * One host round trip (the list sizes, copied into a stack variable) after the census; the
+ * deposit kernels are then enqueued and the call returns: synchronise the stream before reading
+ * grid_dev.  The scratch array is shared by every call in the process on that device and keeps
+ * the last call's contents (what must start at zero is cleared by the call itself): calls that
+ * overlap on the GPU (two streams, two threads) race -- serialise them. */
+#define PSD_STATIC_MAX_N 64
+#define PSD_STATIC_MAX_G 128
+#define PSD_STATIC_MAX_PAIRS (4 << 20)
+#define PSD_STATIC_SCRATCH_BYTES (17 << 20)
+PSD_API int psd_deposit_uniform_static(int device, void* cuda_stream, const void* pos_dev, int dtype,
+                                       int stride_elems, int N, double L, double total_mass, int G,
+                                       double* grid_dev, int64_t* n_pairs_out, char* err, int err_len);
+
 /* Library identification: "libpsd sm_100a <build date>" */
 PSD_API const char* psd_version(void);
 

@@ -9,5 +9,5 @@ from .binding import (  # noqa: F401
     OPT_PATCH_RESTRICT, OPT_PAIR_RECORDS, OPT_ROWS_FP32,
     SUBBLOCK_UNIT,
     RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN, PsdError, PsdStats, Context, lib, version,
-    EXPORTS,
+    EXPORTS, psd_deposit_uniform_static, STATIC_MAX_N, STATIC_MAX_G, STATIC_MAX_PAIRS,
 )

@@ -22,7 +22,7 @@ EXPORTS = ("psd_create", "psd_destroy", "psd_build_tets", "psd_deposit_uniform",
            "psd_refine_patches", "psd_deposit_patches", "psd_deposit_uniform_host",
            "psd_deposit_patches_host",
            "psd_get_stats", "psd_get_tile_counts", "psd_get_tile_class_counts", "psd_set_option", "psd_sync", "psd_last_error", "psd_launch_count",
-           "psd_version")
+           "psd_version", "psd_deposit_uniform_static")
 
 
 class PsdError(RuntimeError):
@@ -94,6 +94,7 @@ def lib() -> C.CDLL:
     L.psd_launch_count.restype = i64
     L.psd_version.argtypes = []
     L.psd_version.restype = C.c_char_p
+    L.psd_deposit_uniform_static.argtypes = [i, vp, vp, i, i, i, d, d, i, vp, C.POINTER(i64), C.c_char_p, i]
     _lib = L
     return L
 
@@ -117,6 +118,30 @@ def _pos_meta(pos):
     if N * N * N != n3 or stride not in (3, 4):
         raise ValueError("positions must hold N^3 particles of 3 or 4 components")
     return dt, stride, N
+
+
+STATIC_MAX_N, STATIC_MAX_G, STATIC_MAX_PAIRS = 64, 128, 4 << 20
+
+
+def psd_deposit_uniform_static(pos_dev, G: int, grid_dev, L: float = 1.0, total_mass: float = 1.0,
+                               device: int = 0, stream=None) -> int:
+    """include/psd.h psd_deposit_uniform_static: the deposit that allocates nothing (no context, all
+    scratch in the library's static device array).  `grid_dev` is the caller's; returns n_pairs."""
+    import torch
+    if not pos_dev.is_cuda or not pos_dev.is_contiguous():
+        raise ValueError("pos_dev must be a contiguous CUDA tensor")
+    if (not grid_dev.is_cuda or grid_dev.dtype != torch.float64 or grid_dev.numel() != G ** 3
+            or not grid_dev.is_contiguous()):
+        raise ValueError("grid_dev must be a contiguous CUDA float64 tensor of G^3 elements")
+    dt, stride, N = _pos_meta(pos_dev)
+    st = stream if stream is not None else torch.cuda.current_stream(device)
+    err = C.create_string_buffer(256)
+    n_pairs = C.c_int64(0)
+    rc = lib().psd_deposit_uniform_static(int(device), C.c_void_p(st.cuda_stream), pos_dev.data_ptr(), dt, stride, N,
+                                          L, total_mass, G, grid_dev.data_ptr(), C.byref(n_pairs), err, 256)
+    if rc:
+        raise PsdError(rc, err.value.decode())
+    return n_pairs.value
 
 
 class Context:

@@ -4,7 +4,9 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstddef>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -872,6 +874,181 @@ int psd_sync(psd_ctx* ctx) {
 const char* psd_last_error(const psd_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
 
 int64_t psd_launch_count(const psd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"
+
+// ---------------------------------------------------------------- a deposit that allocates nothing
+// psd_deposit_uniform_static (include/psd.h): the binned path with every scratch buffer in one
+// file-scope device array.  In host code `psd_static_scratch` is only the host-side stand-in of
+// the symbol, not a device address: the address is asked for once per device (with that device
+// current) with cudaGetSymbolAddress and that pointer is what the kernels are given.
+namespace {
+
+constexpr int STATIC_MAX_TILES = (PSD_STATIC_MAX_G / TILE) * (PSD_STATIC_MAX_G / TILE) * (PSD_STATIC_MAX_G / TILE);
+constexpr int STATIC_MAX_BINS = STATIC_MAX_TILES * N_CLASSES;
+constexpr unsigned int STATIC_CHUNK = 2048;
+constexpr int STATIC_MAX_ITEMS = STATIC_MAX_TILES + PSD_STATIC_MAX_PAIRS / (int)STATIC_CHUNK;
+constexpr int STATIC_MAX_PARTS = (STATIC_MAX_BINS + SCAN_BLOCK - 1) / SCAN_BLOCK;
+
+struct StaticScratch {
+    // cleared at the start of every call (one memset): counts, cursors, statistics
+    unsigned int tile_counts[STATIC_MAX_BINS];
+    unsigned int cursors[STATIC_MAX_BINS];
+    unsigned long long stats[ST_COUNT];
+    unsigned long long hist[128];
+    // written in full by the call before they are read
+    unsigned long long totals[2];
+    unsigned long long part_pairs[STATIC_MAX_PARTS];
+    unsigned long long part_items[STATIC_MAX_PARTS];
+    unsigned long long tile_offsets[STATIC_MAX_BINS + 1];
+    unsigned long long item_offsets[STATIC_MAX_BINS + 1];
+    Item items[STATIC_MAX_ITEMS];
+    unsigned int pair_ids[PSD_STATIC_MAX_PAIRS];
+};
+static_assert(sizeof(StaticScratch) <= (size_t)PSD_STATIC_SCRATCH_BYTES, "scratch layout exceeds the stated size");
+static_assert(offsetof(StaticScratch, totals) % 8 == 0 && offsetof(StaticScratch, items) % 8 == 0, "alignment");
+
+static __device__ __align__(256) unsigned char psd_static_scratch[PSD_STATIC_SCRATCH_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+StaticScratch* g_static_ptr[STATIC_MAX_DEVICES] = {};  // device address of the array, per device
+std::mutex g_static_mutex;
+
+int static_fail(char* err, int err_len, int code, const char* msg) {
+    if (err && err_len > 0) std::snprintf(err, (size_t)err_len, "%s", msg);
+    return code;
+}
+int static_cuda_fail(char* err, int err_len, cudaError_t e, const char* what) {
+    char buf[320];
+    std::snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
+    return static_fail(err, err_len, PSD_ERR_CUDA, buf);
+}
+#define SCK(call)                                                                \
+    do {                                                                         \
+        cudaError_t _e = (call);                                                 \
+        if (_e != cudaSuccess) return static_cuda_fail(err, err_len, _e, #call); \
+    } while (0)
+
+// once per device, with that device current: the array's device address, and the deposit
+// kernel's dynamic shared-memory limit (neither allocates)
+int static_setup(int device, StaticScratch** out, char* err, int err_len) {
+    try {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[device]) {
+            void* ptr = nullptr;
+            SCK(cudaGetSymbolAddress(&ptr, psd_static_scratch));
+            SCK(cudaFuncSetAttribute(k_deposit_tiles<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     DEP_SMEM_BYTES));
+            g_static_ptr[device] = reinterpret_cast<StaticScratch*>(ptr);
+        }
+        *out = g_static_ptr[device];
+    } catch (...) {
+        return static_fail(err, err_len, PSD_ERR_CUDA, "psd_deposit_uniform_static: set-up lock failed");
+    }
+    return PSD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int psd_deposit_uniform_static(int device, void* cuda_stream, const void* pos_dev, int dtype, int stride_elems,
+                               int N, double L, double total_mass, int G, double* grid_dev, int64_t* n_pairs_out,
+                               char* err, int err_len) {
+    if (err && err_len > 0) err[0] = 0;
+    if (n_pairs_out) *n_pairs_out = 0;
+    if (!pos_dev || !grid_dev) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "pos_dev or grid_dev is NULL");
+    if (dtype != PSD_F32 && dtype != PSD_F64) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "dtype must be PSD_F32 or PSD_F64");
+    if (stride_elems != 3 && stride_elems != 4) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "stride_elems must be 3 or 4");
+    if (dtype == PSD_F32 && stride_elems == 4 && (reinterpret_cast<uintptr_t>(pos_dev) & 15))
+        return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "float4 positions must be 16-byte aligned");
+    if (!(L > 0.0) || !std::isfinite(L)) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "L must be finite and > 0");
+    if (!std::isfinite(total_mass)) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "total_mass must be finite");
+    char msg[200];
+    if (N < 2 || N > PSD_STATIC_MAX_N) {
+        std::snprintf(msg, sizeof(msg), "psd_deposit_uniform_static: N = %d is outside [2, %d] (PSD_STATIC_MAX_N; the static scratch is sized for it)", N, PSD_STATIC_MAX_N);
+        return static_fail(err, err_len, PSD_ERR_INVALID_ARG, msg);
+    }
+    if (G < TILE || G > PSD_STATIC_MAX_G || G % TILE) {
+        std::snprintf(msg, sizeof(msg), "psd_deposit_uniform_static: G = %d must be a multiple of 8 in [8, %d] (PSD_STATIC_MAX_G; the static scratch is sized for it)", G, PSD_STATIC_MAX_G);
+        return static_fail(err, err_len, PSD_ERR_INVALID_ARG, msg);
+    }
+    int ndev = 0;
+    SCK(cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev || device >= STATIC_MAX_DEVICES) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "no such device");
+    SCK(cudaSetDevice(device));
+    StaticScratch* sc = nullptr;
+    int rc = static_setup(device, &sc, err, err_len);
+    if (rc) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+    Particles part{};
+    part.pos = pos_dev; part.dtype = dtype; part.stride = stride_elems; part.N = N; part.L = L;
+    {
+        int e = 0;
+        part.inv_L = std::frexp(L, &e) == 0.5 ? 1.0 / L : 0.0;  // exact reciprocal of a power of two
+    }
+    Space space{};
+    space.patch_mode = 0; space.G = G; space.nt = G / TILE; space.out = grid_dev; space.L = L;
+    space.class_small_max = CLASS_SMALL_MAX_CELLS;
+    const long long ncell = (long long)N * N * N;
+    const long long n_tiles = (long long)space.nt * space.nt * space.nt, n_bins = n_tiles * N_CLASSES;
+    const int nparts = (int)((n_bins + SCAN_BLOCK - 1) / SCAN_BLOCK);
+
+    // the array keeps the last call's contents: clear what must start at zero (counts, cursors,
+    // statistics: the head of the layout up to `totals`); the rest is written before it is read
+    SCK(cudaMemsetAsync(sc, 0, offsetof(StaticScratch, totals), st));
+    SCK(cudaMemsetAsync(grid_dev, 0, sizeof(double) * (size_t)G * G * G, st));
+    k_validate<<<1184, 256, 0, st>>>(part, sc->stats);
+    const int cb = 256;
+    const unsigned int cgrid = (unsigned int)((ncell + cb - 1) / cb);
+    k_census<false><<<cgrid, cb, 0, st>>>(part, space, sc->tile_counts, nullptr, nullptr, nullptr, sc->stats, sc->hist);
+    k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(sc->tile_counts, n_bins, STATIC_CHUNK, sc->part_pairs, sc->part_items);
+    k_scan_top<<<1, SCAN_BLOCK, 0, st>>>(sc->part_pairs, sc->part_items, nparts, sc->totals);
+    k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(sc->tile_counts, n_bins, STATIC_CHUNK, sc->part_pairs, sc->part_items,
+                                               sc->tile_offsets, sc->item_offsets);
+    SCK(cudaGetLastError());
+    // the one host round trip: list sizes and the non-finite count, into stack variables
+    unsigned long long totals[2] = {0ull, 0ull}, nonfinite = 0ull;
+    SCK(cudaMemcpyAsync(totals, sc->totals, sizeof(totals), cudaMemcpyDeviceToHost, st));
+    SCK(cudaMemcpyAsync(&nonfinite, sc->stats + ST_NONFINITE, sizeof(nonfinite), cudaMemcpyDeviceToHost, st));
+    SCK(cudaStreamSynchronize(st));
+    if (nonfinite) return static_fail(err, err_len, PSD_ERR_INVALID_ARG, "positions contain NaN or Inf");
+    const unsigned long long n_pairs = totals[0], n_items = totals[1];
+    if (n_pairs_out) *n_pairs_out = (int64_t)n_pairs;
+    if (n_pairs > (unsigned long long)PSD_STATIC_MAX_PAIRS || n_items > (unsigned long long)STATIC_MAX_ITEMS) {
+        std::snprintf(msg, sizeof(msg), "psd_deposit_uniform_static: %llu (tet, tile) pairs exceed PSD_STATIC_MAX_PAIRS = %d (the static pair list); use psd_deposit_uniform",
+                      n_pairs, PSD_STATIC_MAX_PAIRS);
+        return static_fail(err, err_len, PSD_ERR_INVALID_ARG, msg);
+    }
+    if (n_pairs == 0) return PSD_OK;
+    k_items<<<(unsigned int)((n_tiles + 255) / 256), 256, 0, st>>>(sc->tile_counts, n_tiles, STATIC_CHUNK, sc->tile_offsets,
+                                                                  sc->item_offsets, sc->items);
+    k_census<true><<<cgrid, cb, 0, st>>>(part, space, nullptr, sc->tile_offsets, sc->cursors, sc->pair_ids, nullptr, nullptr);
+    DepositArgs A{};
+    A.part = part;
+    A.space = space;
+    A.pair_ids = sc->pair_ids;
+    A.items = sc->items;
+    A.mass_per_tet = total_mass / (6.0 * (double)ncell);
+    A.weight_mode = 0;
+    A.chord_axis = -1;
+    A.stats = sc->stats;
+    A.rec_g = nullptr;  // no pair records: the deposit kernel runs stage A itself
+    A.rec_pair_begin = 0ull;
+    {
+        // fixed-point unit of the tile accumulators, as in run_binned: 2^61 / (chunk x mass of a tet)
+        const double unit = std::fabs(A.mass_per_tet);
+        int eu = 0, ec = 0;
+        if (unit > 0.0 && std::isfinite(unit)) std::frexp(unit, &eu);
+        std::frexp((double)STATIC_CHUNK, &ec);
+        A.acc_scale = std::ldexp(1.0, 61 - eu - ec);
+        A.acc_inv_scale = std::ldexp(1.0, -(61 - eu - ec));
+    }
+    k_deposit_tiles<false, false><<<(unsigned int)n_items, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
+    SCK(cudaGetLastError());
+    return PSD_OK;
+}
 
 const char* psd_version(void) { return "libpsd sm_100a " __DATE__; }
 
