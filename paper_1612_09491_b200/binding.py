@@ -13,7 +13,7 @@ import numpy as np
 from . import _build
 
 F32, F64 = 0, 1
-OPT_WEIGHT_MODE, OPT_KERNEL, OPT_COUNTERS, OPT_CHUNK, OPT_CHORD_AXIS, OPT_REFINE_SUBBLOCK, OPT_CLASS_SMALL_CELLS, OPT_PATCH_RESTRICT, OPT_PAIR_RECORDS, OPT_ROWS_FP32 = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_WEIGHT_MODE, OPT_KERNEL, OPT_COUNTERS, OPT_CHUNK, OPT_CHORD_AXIS, OPT_REFINE_SUBBLOCK, OPT_CLASS_SMALL_CELLS, OPT_PATCH_RESTRICT, OPT_PAIR_RECORDS, OPT_ROWS_FP32, OPT_FACE_SHARING = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 SUBBLOCK_UNIT = 1 << 20
 RULE_LITERAL_TOP_DOWN, RULE_BOTTOM_UP_LEVEL_MEAN = 0, 1
 
@@ -43,7 +43,7 @@ class PsdStats(C.Structure):
         ("n_nonfinite", C.c_int64),
         ("hist_tet", C.c_uint64 * 64), ("hist_pair", C.c_uint64 * 64),
         ("n_face_jobs", C.c_int64), ("n_face_clips", C.c_int64), ("n_plane_evals", C.c_int64),
-        ("n_cells_written", C.c_int64), ("n_restricted_patches", C.c_int64), ("n_general_clips", C.c_int64), ("n_rows_missed", C.c_int64),
+        ("n_cells_written", C.c_int64), ("n_restricted_patches", C.c_int64), ("n_general_clips", C.c_int64), ("n_unit_pairs", C.c_int64), ("n_rows_missed", C.c_int64),
         ("tile_counts_dev", C.c_void_p),
         ("ms_census", C.c_float), ("ms_scan", C.c_float), ("ms_scatter", C.c_float),
         ("ms_deposit", C.c_float), ("ms_total", C.c_float),

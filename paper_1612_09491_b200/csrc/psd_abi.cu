@@ -13,6 +13,7 @@
 
 #include "../../include/psd.h"
 #include "psd_kernels.cuh"
+#include "psd_faces.cuh"
 
 using namespace psd;
 
@@ -49,12 +50,14 @@ struct psd_ctx {
     bool built = false;
     double total_mass = 0.0;
     int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1,
-        use_records = 1, rows_fp32 = 1;
+        use_records = 1, rows_fp32 = 1, face_sharing = 0, face_axis = 2;
+    bool accumulate_now = false;  // the running deposit adds to the caller's grid
     unsigned long long rec_pairs_max = 48ull << 20;  // capacity of the pair-record buffer (REC_PAIRS_MAX)
     long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 2048;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
-        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families, records, slab_bounds;
+        totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families, records, slab_bounds,
+        unit_counts;
     unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
     psd_stats last{};
     bool stats_pending = false;
@@ -131,55 +134,91 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                           nullptr, nullptr, ctx->stats.as<unsigned long long>(),
                                           ctx->hist.as<unsigned long long>());
     CK(cudaEventRecord(ctx->ev[1], st));
-    k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_bins, ctx->chunk,
-                                                   ctx->part_pairs.as<unsigned long long>(),
-                                                   ctx->part_items.as<unsigned long long>());
-    k_scan_top<<<1, SCAN_BLOCK, 0, st>>>(ctx->part_pairs.as<unsigned long long>(),
-                                         ctx->part_items.as<unsigned long long>(), nparts,
-                                         ctx->totals.as<unsigned long long>());
-    k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(ctx->tile_counts.as<unsigned int>(), n_bins, ctx->chunk,
-                                                ctx->part_pairs.as<unsigned long long>(),
-                                                ctx->part_items.as<unsigned long long>(),
-                                                ctx->tile_offsets.as<unsigned long long>(),
-                                                ctx->item_offsets.as<unsigned long long>());
-    ctx->launches += 4;
-    CK(cudaGetLastError());
-    // the only host round trip of a deposit: list sizes, to size the scratch and the grid
-    CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 128, ctx->totals.p, sizeof(unsigned long long) * 2,
-                       cudaMemcpyDeviceToHost, st));
-    // host-output mode (uniform grid): the first work item of each slab of x-tiles
+    // exclusive scan of the per-bin counts (pairs and work items) and the one host round trip of a
+    // binned deposit: list sizes, the slabs' first items (host-output mode), max_extent
     int n_slabs = 0;
-    if (ctx->stream_out_host && !space.patch_mode) {
-        // few slabs for small grids: every launch ends in a partly filled wave
-        n_slabs = space.nt / 8 < 1 ? 1 : (space.nt / 8 < psd_ctx::MAX_SLABS ? space.nt / 8 : psd_ctx::MAX_SLABS);
-        for (int sl = 1; sl < n_slabs; ++sl) {
-            const long long bin = (long long)(sl * space.nt / n_slabs) * space.nt * space.nt * N_CLASSES;
-            CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + sl, ctx->item_offsets.as<unsigned long long>() + bin,
-                               sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-            CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + psd_ctx::MAX_SLABS + 1 + sl,
-                               ctx->tile_offsets.as<unsigned long long>() + bin, sizeof(unsigned long long),
-                               cudaMemcpyDeviceToHost, st));
+    auto scan_and_sync = [&](const unsigned int* counts) -> int {
+        k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(counts, n_bins, ctx->chunk, ctx->part_pairs.as<unsigned long long>(),
+                                                       ctx->part_items.as<unsigned long long>());
+        k_scan_top<<<1, SCAN_BLOCK, 0, st>>>(ctx->part_pairs.as<unsigned long long>(),
+                                             ctx->part_items.as<unsigned long long>(), nparts,
+                                             ctx->totals.as<unsigned long long>());
+        k_scan_final<<<nparts, SCAN_BLOCK, 0, st>>>(counts, n_bins, ctx->chunk, ctx->part_pairs.as<unsigned long long>(),
+                                                    ctx->part_items.as<unsigned long long>(),
+                                                    ctx->tile_offsets.as<unsigned long long>(),
+                                                    ctx->item_offsets.as<unsigned long long>());
+        ctx->launches += 3;
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 128, ctx->totals.p, sizeof(unsigned long long) * 2,
+                           cudaMemcpyDeviceToHost, st));
+        // host-output mode (uniform grid): the first work item of each slab of x-tiles
+        n_slabs = 0;
+        if (ctx->stream_out_host && !space.patch_mode) {
+            // few slabs for small grids: every launch ends in a partly filled wave
+            n_slabs = space.nt / 8 < 1 ? 1 : (space.nt / 8 < psd_ctx::MAX_SLABS ? space.nt / 8 : psd_ctx::MAX_SLABS);
+            for (int sl = 1; sl < n_slabs; ++sl) {
+                const long long bin = (long long)(sl * space.nt / n_slabs) * space.nt * space.nt * N_CLASSES;
+                CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + sl, ctx->item_offsets.as<unsigned long long>() + bin,
+                                   sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+                CK(cudaMemcpyAsync(ctx->pinned + ST_COUNT + 130 + psd_ctx::MAX_SLABS + 1 + sl,
+                                   ctx->tile_offsets.as<unsigned long long>() + bin, sizeof(unsigned long long),
+                                   cudaMemcpyDeviceToHost, st));
+            }
         }
-    }
-    CK(cudaMemcpyAsync(ctx->pinned + ST_MAX_EXTENT, ctx->stats.as<unsigned long long>() + ST_MAX_EXTENT,
-                       sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    const unsigned long long n_pairs = ctx->pinned[ST_COUNT + 128], n_items = ctx->pinned[ST_COUNT + 129];
+        CK(cudaMemcpyAsync(ctx->pinned + ST_MAX_EXTENT, ctx->stats.as<unsigned long long>() + ST_MAX_EXTENT,
+                           sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return PSD_OK;
+    };
+    ctx->launches += 1;
+    rc = scan_and_sync(ctx->tile_counts.as<unsigned int>());
+    if (rc) return rc;
+    unsigned long long n_pairs = ctx->pinned[ST_COUNT + 128], n_items = ctx->pinned[ST_COUNT + 129];
     const unsigned long long max_extent = ctx->pinned[ST_MAX_EXTENT];  // largest cell range of a tet along an axis (level 0)
     ctx->last.n_pairs = (int64_t)n_pairs;
     ctx->last.n_work_items = (int64_t)n_items;
     ctx->last.n_tiles = n_tiles;
     CK(cudaEventRecord(ctx->ev[2], st));
+    // Shared faces (psd_faces.cuh): every face of the tessellation clipped once for its two tets.
+    // Uniform grids, not accumulating (the grid is in fixed point until the end), every unit (two
+    // tets) plus a tile shorter than the grid (one periodic image per pair), 32-bit unit ids.
+    const bool face_mode = ctx->face_sharing && ctx->use_records && !space.patch_mode && !ctx->accumulate_now &&
+                           n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G &&
+                           (long long)FACE_UNITS * ncell < 4294967296ll;
+    const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_axis;
+    const unsigned int ugrid = (unsigned int)((ncell * FACE_UNITS + FCENSUS_THREADS - 1) / FCENSUS_THREADS);
+    const unsigned int* bin_counts = ctx->tile_counts.as<unsigned int>();
+    if (face_mode) {
+        // the units' own census (the tet census above stays: statistics, tile_counts, max_extent)
+        CK(ctx->unit_counts.ensure(sizeof(unsigned int) * n_bins));
+        CK(cudaMemsetAsync(ctx->unit_counts.p, 0, sizeof(unsigned int) * n_bins, st));
+        k_face_census<false><<<ugrid, FCENSUS_THREADS, 0, st>>>(ctx->part, space, face_axis, ctx->weight_mode,
+                                                                ctx->unit_counts.as<unsigned int>(), nullptr, nullptr, nullptr);
+        ctx->launches += 1;
+        bin_counts = ctx->unit_counts.as<unsigned int>();
+        rc = scan_and_sync(bin_counts);
+        if (rc) return rc;
+        n_pairs = ctx->pinned[ST_COUNT + 128];
+        n_items = ctx->pinned[ST_COUNT + 129];
+        ctx->last.n_work_items = (int64_t)n_items;
+        ctx->last.n_unit_pairs = (int64_t)n_pairs;
+    }
     if (n_pairs > 0) {
         if (n_items > 0x7fffffffull) return fail(ctx, PSD_ERR_INVALID_ARG, "too many work items");
         CK(ctx->pair_ids.ensure(sizeof(unsigned int) * n_pairs));
         CK(ctx->items.ensure(sizeof(Item) * n_items));
         k_items<<<(unsigned int)((n_tiles + 255) / 256), 256, 0, st>>>(
-            ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
+            bin_counts, n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
             ctx->item_offsets.as<unsigned long long>(), ctx->items.as<Item>());
-        k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
-                                             ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
-                                             nullptr, nullptr);
+        if (face_mode)
+            k_face_census<true><<<ugrid, FCENSUS_THREADS, 0, st>>>(ctx->part, space, face_axis, ctx->weight_mode, nullptr,
+                                                                   ctx->tile_offsets.as<unsigned long long>(),
+                                                                   ctx->cursors.as<unsigned int>(),
+                                                                   ctx->pair_ids.as<unsigned int>());
+        else
+            k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
+                                                 ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
+                                                 nullptr, nullptr);
         ctx->launches += 2;
         CK(cudaEventRecord(ctx->ev[3], st));
         DepositArgs A{};
@@ -202,6 +241,17 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.acc_scale = std::ldexp(1.0, 61 - eu - ec);
             A.acc_inv_scale = std::ldexp(1.0, -(61 - eu - ec));
         }
+        if (face_mode) {
+            // tiles and grid are summed modulo 2^64 from end to end: the unit is 2^-62 of a bound of
+            // the FINAL value of a cell (the whole mass; in signed-volume mode every cell ends at 1)
+            A.chord_axis = face_axis;
+            int eb = 0;
+            const double bound = ctx->weight_mode == 0 ? std::fabs(ctx->total_mass) : 2.0;
+            if (bound > 0.0 && std::isfinite(bound)) std::frexp(bound, &eb);  // bound < 2^eb
+            A.acc_scale = std::ldexp(1.0, 62 - eb);
+            A.acc_inv_scale = std::ldexp(1.0, -(62 - eb));
+        }
+        const size_t rec_bytes = face_mode ? sizeof(double) * FREC_DOUBLES : REC_BYTES;
         // ---- launch ranges of work items.  Boundaries (item index, first pair): the slabs of x-tiles
         // whose part of the grid goes back to the host while later slabs are deposited (host-output
         // mode), and the slabs of the pair-record buffer (k_pair_records writes the records of a
@@ -219,7 +269,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         unsigned long long rec_cap = 0;
         if (ctx->use_records) {
             const unsigned long long want = n_pairs < ctx->rec_pairs_max ? n_pairs : ctx->rec_pairs_max;
-            if (ctx->records.ensure((size_t)want * REC_BYTES) == cudaSuccess) rec_cap = want;
+            if (ctx->records.ensure((size_t)want * rec_bytes) == cudaSuccess) rec_cap = want;
             // (no room: the deposit kernel then runs stage A itself)
         }
         if (rec_cap && n_pairs > rec_cap) {
@@ -268,11 +318,20 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         const bool rec_only = rec_cap != 0 && (long long)max_extent + 2 + TILE < g_min;
         const Item* items0 = A.items;
         const size_t plane = sizeof(double) * (size_t)space.G * space.G;
+        if (face_mode && !rec_cap)
+            return fail(ctx, PSD_ERR_OOM, "no room for the pair records of the shared-face path (PSD_OPT_FACE_SHARING = 0 runs without)");
         for (int i = 0; i + 1 < nb; ++i) {
             const unsigned long long cnt = bounds[i + 1].item - bounds[i].item;
             if (cnt) {
                 A.items = items0 + bounds[i].item;
                 A.rec_pair_begin = bounds[i].pair;
+                if (face_mode) {
+                    if (ctx->rows_fp32) k_face_records<1><<<(unsigned int)cnt, FREC_THREADS, 0, st>>>(A);
+                    else k_face_records<0><<<(unsigned int)cnt, FREC_THREADS, 0, st>>>(A);
+                    if (ctx->counters) k_deposit_faces<true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
+                    else k_deposit_faces<false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
+                    ctx->launches += 2;
+                } else {
                 if (rec_cap) {
                     if (ctx->rows_fp32 && ctx->counters) k_pair_records<2><<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
                     else if (ctx->rows_fp32) k_pair_records<1><<<(unsigned int)cnt, REC_THREADS, 0, st>>>(A);
@@ -287,8 +346,15 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                     else k_deposit_tiles<false, false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES, st>>>(A);
                 }
                 ctx->launches += 1;
+                }
             }
             const int sl = bounds[i + 1].x_slab_end;
+            if (sl >= 0 && face_mode) {  // the slab's planes from fixed point to fp64 before they leave
+                const size_t x0 = (size_t)(sl * space.nt / n_slabs) * TILE, x1 = (size_t)((sl + 1) * space.nt / n_slabs) * TILE;
+                k_fixed_to_double<<<1184, 256, 0, st>>>(space.out + x0 * (size_t)space.G * space.G,
+                                                        (long long)((x1 - x0) * (size_t)space.G * space.G), A.acc_inv_scale);
+                ctx->launches += 1;
+            }
             if (sl >= 0) {  // a slab of x-tiles is complete: its part of the grid goes to the host
                 CK(cudaEventRecord(ctx->slab_ev[sl], st));
                 CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_ev[sl], 0));
@@ -297,6 +363,10 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                    reinterpret_cast<const char*>(space.out) + x0 * plane, (x1 - x0) * plane,
                                    cudaMemcpyDeviceToHost, ctx->copy_stream));
             }
+        }
+        if (face_mode && n_slabs <= 1) {
+            k_fixed_to_double<<<1184, 256, 0, st>>>(space.out, (long long)space.G * space.G * space.G, A.acc_inv_scale);
+            ctx->launches += 1;
         }
         if (n_slabs > 1) {
             CK(cudaEventRecord(ctx->copy_done, ctx->copy_stream));
@@ -383,6 +453,10 @@ int psd_create(psd_ctx** out, int device, void* cuda_stream) {
         e = cudaFuncSetAttribute(k_deposit_tiles<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_deposit_tiles<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_faces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_deposit_faces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
     if (e != cudaSuccess) {
         psd_destroy(ctx);
         return PSD_ERR_CUDA;
@@ -397,7 +471,7 @@ void psd_destroy(psd_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->tile_counts, &ctx->cursors, &ctx->tile_offsets, &ctx->item_offsets, &ctx->items,
                       &ctx->pair_ids, &ctx->part_pairs, &ctx->part_items, &ctx->totals, &ctx->stats, &ctx->hist,
-                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families, &ctx->records, &ctx->slab_bounds};
+                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families, &ctx->records, &ctx->slab_bounds, &ctx->unit_counts};
     for (DevBuf* b : bufs) b->release();
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 6; ++i)
@@ -456,6 +530,7 @@ int psd_deposit_uniform(psd_ctx* ctx, int G, double* grid_dev, int accumulate) {
     if (!grid_dev) return fail(ctx, PSD_ERR_INVALID_ARG, "grid_dev is NULL");
     CK(cudaSetDevice(ctx->device));
     if (!accumulate) CK(cudaMemsetAsync(grid_dev, 0, sizeof(double) * (size_t)G * G * G, ctx->stream));
+    ctx->accumulate_now = accumulate != 0;
     Space s{};
     s.patch_mode = 0;
     s.G = G;
@@ -849,6 +924,11 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
             if (value < 0.0 || value > 4e9) return fail(ctx, PSD_ERR_INVALID_ARG, "pair records: 0, 1 or a capacity in pairs");
             ctx->use_records = value != 0.0;
             ctx->rec_pairs_max = value > 1.0 ? (unsigned long long)value : REC_PAIRS_MAX;
+            return PSD_OK;
+        case PSD_OPT_FACE_SHARING:
+            if (iv < 0 || iv > 3) return fail(ctx, PSD_ERR_INVALID_ARG, "face sharing: 0 (off) or 1 + chord axis (1..3)");
+            ctx->face_sharing = iv != 0;
+            if (iv) ctx->face_axis = iv - 1;
             return PSD_OK;
         case PSD_OPT_ROWS_FP32:
             if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "fp32 rows must be 0 or 1");
