@@ -93,15 +93,15 @@ enum {
                                 margin of 1e-9 (0).  Either set holds every column with a non-empty
                                 polygon and the clip itself is fp64, so the deposit is the same;
                                 fp32 admits a few more empty jobs (n_face_jobs).               */
-    PSD_OPT_FACE_SHARING = 10, /* binned path, uniform grids.  0 (default): the tet formulation.
-                                1..3: every face of the tessellation is clipped ONCE for the two
-                                tets that share it, along one chord axis for the whole deposit
-                                (value - 1 = x / y / z, unless PSD_OPT_CHORD_AXIS fixes one); units
-                                = the 12 faces a Lagrangian cell owns, binned by tile on their own;
-                                tiles and grid are summed in 64-bit fixed point and converted to
-                                fp64 at the end.  Runs when twice the largest cell range of a tet
-                                plus a tile fits the grid and accumulate = 0, else the tet
-                                formulation does.  Measured slower as a whole.    */
+    PSD_OPT_FACE_SHARING = 10, /* binned path, uniform grids.  1..3 (default 1): every face of the
+                                tessellation is clipped ONCE, for the two tets that share it, in
+                                the (tet, tile) pair of the tet that owns it; one chord axis for
+                                the whole deposit (value - 1 = x / y / z, unless
+                                PSD_OPT_CHORD_AXIS fixes one); tiles and grid are summed in 64-bit
+                                fixed point (unit 2^-62 of the total mass) and converted to fp64 at
+                                the end.  Runs when twice the largest cell range of a tet plus a
+                                tile fits the grid, with pair records and accumulate = 0; else,
+                                and with 0, the tet formulation runs (stats.shared_faces).     */
     PSD_OPT_PATCH_RESTRICT = 7  /* psd_deposit_patches, PAPER.md:193 (coarser representations of the
                                 internal nodes).  1 (default): a listed patch whose 8 children are
                                 all listed too is not deposited into; it is filled afterwards by
@@ -147,8 +147,8 @@ typedef struct {
     int64_t n_restricted_patches; /* psd_deposit_patches: patches filled from their children     */
     int64_t n_general_clips; /* counters: face jobs the straight-line clip passed to the general
                                convex clip (a tie within its margin: lattice-aligned input)  */
-    int64_t n_unit_pairs;    /* shared-face path: (face unit, tile) pairs of the last deposit (0: the
-                               tet formulation ran)                                            */
+    int64_t shared_faces;    /* 1: the last deposit clipped every face once for its two tets
+                               (PSD_OPT_FACE_SHARING), 0: the tet formulation ran              */
     int64_t n_rows_missed;   /* counters, PSD_OPT_ROWS_FP32 = 1: rows of faces whose fp64 column range
                                the fp32 classification does not cover (a self-check: 0)       */
     /* device pointer to the per-(tile, size class) pair counts of the last binned deposit

@@ -43,7 +43,7 @@ class PsdStats(C.Structure):
         ("n_nonfinite", C.c_int64),
         ("hist_tet", C.c_uint64 * 64), ("hist_pair", C.c_uint64 * 64),
         ("n_face_jobs", C.c_int64), ("n_face_clips", C.c_int64), ("n_plane_evals", C.c_int64),
-        ("n_cells_written", C.c_int64), ("n_restricted_patches", C.c_int64), ("n_general_clips", C.c_int64), ("n_unit_pairs", C.c_int64), ("n_rows_missed", C.c_int64),
+        ("n_cells_written", C.c_int64), ("n_restricted_patches", C.c_int64), ("n_general_clips", C.c_int64), ("shared_faces", C.c_int64), ("n_rows_missed", C.c_int64),
         ("tile_counts_dev", C.c_void_p),
         ("ms_census", C.c_float), ("ms_scan", C.c_float), ("ms_scatter", C.c_float),
         ("ms_deposit", C.c_float), ("ms_total", C.c_float),

@@ -50,14 +50,14 @@ struct psd_ctx {
     bool built = false;
     double total_mass = 0.0;
     int weight_mode = 0, kernel = 0, counters = 0, chord_axis = -1, refine_subblock = 0, patch_restrict = 1,
-        use_records = 1, rows_fp32 = 1, face_sharing = 0, face_axis = 2;
+        use_records = 1, rows_fp32 = 1, face_sharing = 1;
     bool accumulate_now = false;  // the running deposit adds to the caller's grid
     unsigned long long rec_pairs_max = 48ull << 20;  // capacity of the pair-record buffer (REC_PAIRS_MAX)
     long long class_small = CLASS_SMALL_MAX_CELLS;
     unsigned int chunk = 2048;
     DevBuf tile_counts, cursors, tile_offsets, item_offsets, items, pair_ids, part_pairs, part_items,
         totals, stats, hist, patches, lookup, refine_counts, host_pos, host_grid, families, records, slab_bounds,
-        unit_counts, tet_info, tile_axis;
+        tet_info;
     unsigned long long* pinned = nullptr;  // [ST_COUNT + 128 + 2] staging
     psd_stats last{};
     bool stats_pending = false;
@@ -180,48 +180,22 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     ctx->last.n_tiles = n_tiles;
     CK(cudaEventRecord(ctx->ev[2], st));
     // Shared faces (psd_faces.cuh): every face of the tessellation clipped once for its two tets.
-    // Uniform grids, not accumulating (the grid is in fixed point until the end), every unit (two
-    // tets) plus a tile shorter than the grid (one periodic image per pair), 32-bit unit ids.
-    const bool share_ok = ctx->face_sharing && ctx->use_records && !space.patch_mode && !ctx->accumulate_now &&
-                          n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G &&
-                          (long long)FACE_UNITS * ncell < 4294967296ll;
-    const bool face_mode = share_ok && ctx->face_sharing <= 3;   // units with a census of their own
-    const bool pair_share = share_ok && ctx->face_sharing > 3;   // shared faces on the (tet, tile) pairs
-    const bool fixed_grid = face_mode || pair_share;             // the grid is in fixed point until the end
-    const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_axis;
-    const unsigned int ugrid = (unsigned int)((ncell * FACE_UNITS + FCENSUS_THREADS - 1) / FCENSUS_THREADS);
-    const unsigned int* bin_counts = ctx->tile_counts.as<unsigned int>();
-    if (face_mode) {
-        // the units' own census (the tet census above stays: statistics, tile_counts, max_extent)
-        CK(ctx->unit_counts.ensure(sizeof(unsigned int) * n_bins));
-        CK(cudaMemsetAsync(ctx->unit_counts.p, 0, sizeof(unsigned int) * n_bins, st));
-        k_face_census<false><<<ugrid, FCENSUS_THREADS, 0, st>>>(ctx->part, space, face_axis, ctx->weight_mode,
-                                                                ctx->unit_counts.as<unsigned int>(), nullptr, nullptr, nullptr);
-        ctx->launches += 1;
-        bin_counts = ctx->unit_counts.as<unsigned int>();
-        rc = scan_and_sync(bin_counts);
-        if (rc) return rc;
-        n_pairs = ctx->pinned[ST_COUNT + 128];
-        n_items = ctx->pinned[ST_COUNT + 129];
-        ctx->last.n_work_items = (int64_t)n_items;
-        ctx->last.n_unit_pairs = (int64_t)n_pairs;
-    }
+    // Uniform grids, not accumulating (the grid is in fixed point until the end), two tets plus a
+    // tile shorter than the grid (one periodic image per pair, neighbours' ranges unambiguous).
+    const bool pair_share = ctx->face_sharing && ctx->use_records && !space.patch_mode && !ctx->accumulate_now &&
+                            n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G;
+    const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_sharing - 1;
+    ctx->last.shared_faces = pair_share ? 1 : 0;
     if (n_pairs > 0) {
         if (n_items > 0x7fffffffull) return fail(ctx, PSD_ERR_INVALID_ARG, "too many work items");
         CK(ctx->pair_ids.ensure(sizeof(unsigned int) * n_pairs));
         CK(ctx->items.ensure(sizeof(Item) * n_items));
         k_items<<<(unsigned int)((n_tiles + 255) / 256), 256, 0, st>>>(
-            bin_counts, n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
+            ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
             ctx->item_offsets.as<unsigned long long>(), ctx->items.as<Item>());
-        if (face_mode)
-            k_face_census<true><<<ugrid, FCENSUS_THREADS, 0, st>>>(ctx->part, space, face_axis, ctx->weight_mode, nullptr,
-                                                                   ctx->tile_offsets.as<unsigned long long>(),
-                                                                   ctx->cursors.as<unsigned int>(),
-                                                                   ctx->pair_ids.as<unsigned int>());
-        else
-            k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
-                                                 ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
-                                                 nullptr, nullptr);
+        k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
+                                             ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
+                                             nullptr, nullptr);
         ctx->launches += 2;
         CK(cudaEventRecord(ctx->ev[3], st));
         DepositArgs A{};
@@ -244,25 +218,23 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.acc_scale = std::ldexp(1.0, 61 - eu - ec);
             A.acc_inv_scale = std::ldexp(1.0, -(61 - eu - ec));
         }
-        if (fixed_grid) {
+        if (pair_share) {
             // tiles and grid are summed modulo 2^64 from end to end: the unit is 2^-62 of a bound of
             // the FINAL value of a cell (the whole mass; in signed-volume mode every cell ends at 1)
             A.chord_axis = face_axis;
-            A.tile_axis = nullptr;
-            A.tet_info = nullptr;
-            if (pair_share) {
-                CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell)));
-                k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)space.G / space.L, ctx->tet_info.as<TetInfo>());
-                ctx->launches += 1;
-                A.tet_info = ctx->tet_info.p;
-            }
             int eb = 0;
             const double bound = ctx->weight_mode == 0 ? std::fabs(ctx->total_mass) : 2.0;
             if (bound > 0.0 && std::isfinite(bound)) std::frexp(bound, &eb);  // bound < 2^eb
             A.acc_scale = std::ldexp(1.0, 62 - eb);
             A.acc_inv_scale = std::ldexp(1.0, -(62 - eb));
+            // what a pair needs of its tet and the four neighbours: determinant, cell range
+            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell)));
+            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)space.G / space.L,
+                                                                                ctx->tet_info.as<TetInfo>());
+            ctx->launches += 1;
+            A.tet_info = ctx->tet_info.p;
         }
-        const size_t rec_bytes = face_mode ? sizeof(double) * FREC_DOUBLES : (pair_share ? sizeof(double) * REC2_DOUBLES : REC_BYTES);
+        const size_t rec_bytes = pair_share ? sizeof(double) * REC2_DOUBLES : REC_BYTES;
         // ---- launch ranges of work items.  Boundaries (item index, first pair): the slabs of x-tiles
         // whose part of the grid goes back to the host while later slabs are deposited (host-output
         // mode), and the slabs of the pair-record buffer (k_pair_records writes the records of a
@@ -329,20 +301,14 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         const bool rec_only = rec_cap != 0 && (long long)max_extent + 2 + TILE < g_min;
         const Item* items0 = A.items;
         const size_t plane = sizeof(double) * (size_t)space.G * space.G;
-        if (fixed_grid && !rec_cap)
+        if (pair_share && !rec_cap)
             return fail(ctx, PSD_ERR_OOM, "no room for the pair records of the shared-face path (PSD_OPT_FACE_SHARING = 0 runs without)");
         for (int i = 0; i + 1 < nb; ++i) {
             const unsigned long long cnt = bounds[i + 1].item - bounds[i].item;
             if (cnt) {
                 A.items = items0 + bounds[i].item;
                 A.rec_pair_begin = bounds[i].pair;
-                if (face_mode) {
-                    if (ctx->rows_fp32) k_face_records<1><<<(unsigned int)cnt, FREC_THREADS, 0, st>>>(A);
-                    else k_face_records<0><<<(unsigned int)cnt, FREC_THREADS, 0, st>>>(A);
-                    if (ctx->counters) k_deposit_faces<true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
-                    else k_deposit_faces<false><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
-                    ctx->launches += 2;
-                } else if (pair_share) {
+                if (pair_share) {
                     if (ctx->rows_fp32) k_pair_records2<1><<<(unsigned int)cnt, REC2_THREADS, 0, st>>>(A);
                     else k_pair_records2<0><<<(unsigned int)cnt, REC2_THREADS, 0, st>>>(A);
                     if (ctx->counters) k_deposit_tiles2<true><<<(unsigned int)cnt, DEP_THREADS, DEP_SMEM_BYTES_REC, st>>>(A);
@@ -366,7 +332,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                 }
             }
             const int sl = bounds[i + 1].x_slab_end;
-            if (sl >= 0 && fixed_grid) {  // the slab's planes from fixed point to fp64 before they leave
+            if (sl >= 0 && pair_share) {  // the slab's planes from fixed point to fp64 before they leave
                 const size_t x0 = (size_t)(sl * space.nt / n_slabs) * TILE, x1 = (size_t)((sl + 1) * space.nt / n_slabs) * TILE;
                 k_fixed_to_double<<<1184, 256, 0, st>>>(space.out + x0 * (size_t)space.G * space.G,
                                                         (long long)((x1 - x0) * (size_t)space.G * space.G), A.acc_inv_scale);
@@ -381,7 +347,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                    cudaMemcpyDeviceToHost, ctx->copy_stream));
             }
         }
-        if (fixed_grid && n_slabs <= 1) {
+        if (pair_share && n_slabs <= 1) {
             k_fixed_to_double<<<1184, 256, 0, st>>>(space.out, (long long)space.G * space.G * space.G, A.acc_inv_scale);
             ctx->launches += 1;
         }
@@ -471,10 +437,6 @@ int psd_create(psd_ctx** out, int device, void* cuda_stream) {
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_deposit_tiles<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_deposit_faces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_deposit_faces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
-    if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_deposit_tiles2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_deposit_tiles2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DEP_SMEM_BYTES_REC);
@@ -492,7 +454,7 @@ void psd_destroy(psd_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->tile_counts, &ctx->cursors, &ctx->tile_offsets, &ctx->item_offsets, &ctx->items,
                       &ctx->pair_ids, &ctx->part_pairs, &ctx->part_items, &ctx->totals, &ctx->stats, &ctx->hist,
-                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families, &ctx->records, &ctx->slab_bounds, &ctx->unit_counts, &ctx->tet_info, &ctx->tile_axis};
+                      &ctx->patches, &ctx->lookup, &ctx->refine_counts, &ctx->host_pos, &ctx->host_grid, &ctx->families, &ctx->records, &ctx->slab_bounds, &ctx->tet_info};
     for (DevBuf* b : bufs) b->release();
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 6; ++i)
@@ -947,9 +909,8 @@ int psd_set_option(psd_ctx* ctx, int key, double value) {
             ctx->rec_pairs_max = value > 1.0 ? (unsigned long long)value : REC_PAIRS_MAX;
             return PSD_OK;
         case PSD_OPT_FACE_SHARING:
-            if (iv < 0 || iv > 7) return fail(ctx, PSD_ERR_INVALID_ARG, "face sharing: 0 (off), 1..3 (units, axis), 4..6 (pairs, axis), 7 (pairs, axis per tile)");
+            if (iv < 0 || iv > 3) return fail(ctx, PSD_ERR_INVALID_ARG, "face sharing: 0 (off) or 1 + chord axis (1..3)");
             ctx->face_sharing = iv;
-            if (iv >= 1 && iv <= 6) ctx->face_axis = (iv - 1) % 3;
             return PSD_OK;
         case PSD_OPT_ROWS_FP32:
             if (iv != 0 && iv != 1) return fail(ctx, PSD_ERR_INVALID_ARG, "fp32 rows must be 0 or 1");

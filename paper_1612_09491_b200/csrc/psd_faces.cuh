@@ -3,220 +3,35 @@
 // In the tet formulation (psd_kernels.cuh) a tet is its 4 oriented faces and each face job
 // (face x column) adds  w_T * Phi(face; column, cell)  to the cells of the tet's range, Phi being
 // antisymmetric in the orientation of the face.  Every face of the Lagrangian tessellation
-// (PAPER.md:43, the 6 tets of a cell share the cell's main diagonal) belongs to exactly two
-// tets, A and B, which see it with opposite orientations, so one job can serve both:
-//     cell c  +=  ( w_A [c in range of A]  -  w_B [c in range of B] ) * Phi(face; column, c)
-// -- half the clips, polygons and plane integrals.  It needs one chord axis for all tets that
-// add to a column (here: one axis per deposit) where the tet formulation picks the longest axis
-// of each tet, which costs 30-40 % more jobs per face; the halving wins.
+// (PAPER.md:43; the 6 tets of a cell share the cell's main diagonal) belongs to exactly two
+// tets, T and N, which see it with opposite orientations, so one job can serve both:
+//     cell c  +=  ( w_T [c in range of T]  -  w_N [c in range of N] ) * Phi(face; column, c)
+// -- 33 % fewer clips, half the plane integrals and tile adds.  It needs one chord axis for all
+// tets that add to a column (here: one axis per deposit) where the tet formulation picks the
+// longest axis of each tet, which costs 30-40 % more jobs per face; the halving wins.
 //
-// Units: the 12 faces a Lagrangian cell owns -- the 6 that contain its main diagonal (both tets
-// in the cell) and the 6 on its three low sides (tet A in the cell, tet B in the neighbour below);
-// each unit is binned into the 8^3 tiles where it has jobs, one 104-byte record per (unit, tile).
-// A tet that lies inside one cell, or is degenerate, is not deposited through its faces: its
-// mass goes to its cell as a "special" of the unit of its low-side face (every tet has one).
+// The binning stays by (tet, tile) pair.  In the pair (T, X) a face F of T, shared with the
+// neighbour N, is clipped -- once, for both tets -- if T owns F or if N does not meet tile X (then
+// no pair (N, X) exists); it is skipped if N owns it and the pair (N, X) exists, which clips it
+// there.  Every decision is local to the pair: what it needs of the four neighbours (determinant,
+// cell range) comes from a per-tet table written once per deposit (k_tet_info).
+// A tet that lies inside one cell, or is degenerate, is not deposited through its faces: its mass
+// goes to its cell as the pair's "special" (its faces are still clipped where a neighbour needs them).
 //
 // The partial sums of a work item are no longer sums of whole tets, so they are not bounded by
 // the mass of its tets: tiles and grid are accumulated in 64-bit fixed point modulo 2^64 from end
-// to end (unit 2^-k of a bound of the final cell value; integer addition commutes and wraps
+// to end (unit 2^-62 of a bound of the final cell value; integer addition commutes and wraps
 // harmlessly) and the grid is converted to fp64 by a last pass (k_fixed_to_double).
+//
+// Measured and dropped: the same with units = the 12 faces a Lagrangian cell owns, binned by a
+// census of their own (1.9x the pairs, 3.5x the binning cost: slower as a whole); a chord axis per
+// tile chosen from the pairs' column counts (4 % fewer jobs: tets in a tile are not aligned).
 #pragma once
 #include "psd_kernels.cuh"
 
 namespace psd {
 
-// nibbles 0..2: the face's vertices in tet A's orientation, as POSITIONS in tet A's vertex list;
-// nibbles 3..6: tet A, 7..10: tet B (their own vertex order: corner 0, a, b, corner 7 of their
-// cell), as local particle indices: 0..7 the corners of this cell (bit 0 = +x, 1 = +y, 2 = +z),
-// 8 / 9 / 10 the corner 0 of the cell at -x / -y / -z.  Bit 44: a low-side face (owns tet A's
-// special); bits 45..47: tet A's number in its cell.
-// Derived from c_kuhn_mid and FACE_TABLE (every face holds corner 0 of this cell).
-__device__ __constant__ unsigned long long c_face_units[12] = {
-    0x0072307310230ull,  // diagonal face (0, 7, 3): tet 0, tet 2
-    0x0071507310310ull,  // diagonal face (0, 1, 7): tet 0, tet 1
-    0x0275407150310ull,  // diagonal face (0, 5, 7): tet 1, tet 4
-    0x0476207230230ull,  // diagonal face (0, 7, 2): tet 2, tet 3
-    0x0674607620230ull,  // diagonal face (0, 7, 6): tet 3, tet 5
-    0x0874607540310ull,  // diagonal face (0, 4, 7): tet 4, tet 5
-    0x01310a7310120ull,  // low-side face (0, 3, 1): tet 0, tet 4 of the cell at (0, 0, -1)
-    0x0350197150120ull,  // low-side face (0, 1, 5): tet 1, tet 2 of the cell at (0, -1, 0)
-    0x05302a7230120ull,  // low-side face (0, 2, 3): tet 2, tet 5 of the cell at (0, 0, -1)
-    0x0762087620120ull,  // low-side face (0, 6, 2): tet 3, tet 0 of the cell at (-1, 0, 0)
-    0x0954097540120ull,  // low-side face (0, 5, 4): tet 4, tet 3 of the cell at (0, -1, 0)
-    0x0b60487460120ull,  // low-side face (0, 4, 6): tet 5, tet 1 of the cell at (-1, 0, 0)
-};
-
-constexpr int FACE_UNITS = 12;
-__device__ __forceinline__ int unit_nib(unsigned long long w, int i) { return (int)(w >> (4 * i)) & 15; }
-__device__ __forceinline__ bool unit_low_side(unsigned long long w) { return (w >> 44) & 1ull; }
-
-// lattice index of local particle l (0..10) of Lagrangian cell (i, j, k)
-__device__ __forceinline__ int64_t unit_particle(int i, int j, int k, int l, int N) {
-    if (l < 8) return corner_index(i, j, k, l, N);
-    int ii = i, jj = j, kk = k;
-    if (l == 8) ii = i == 0 ? N - 1 : i - 1;
-    else if (l == 9) jj = j == 0 ? N - 1 : j - 1;
-    else kk = k == 0 ? N - 1 : k - 1;
-    return ((int64_t)ii * N + jj) * N + kk;
-}
-
-// What the census and the record kernel must agree on for a unit: the tets' cell ranges, which
-// of them deposit through their faces ("active": not inside one cell, not degenerate), tet A's
-// special (low-side units only), the face's cell rectangle across the chord axis and its top.
-struct UnitBox {
-    int loA[3], hiA[3], loB[3], hiB[3];
-    bool actA, actB;
-    bool special;          // tet A goes whole to one cell
-    int scell[3];          // that cell (grid units, unwrapped)
-    bool degenerate;       // tet A has determinant 0 (its special is its centroid cell, mass mode only)
-    int v0, v1, w0, w1;    // columns the face's projection can meet: floor(min) .. ceil(max) - 1
-    int utop, ulo;         // highest cell below the face's top; lowest cell of the active tets
-};
-// gA, gB: the tets' vertices (grid units, unwrapped to one image); fp: positions of the face's
-// vertices in gA.  ax: chord axis.
-__device__ __forceinline__ UnitBox unit_box(const double gA[4][3], const double gB[4][3], const int fp[3],
-                                            const bool low_side, const int ax, const int weight_mode) {
-    UnitBox b;
-#pragma unroll
-    for (int x = 0; x < 3; ++x) {
-        b.loA[x] = __double2int_rd(fmin(fmin(gA[0][x], gA[1][x]), fmin(gA[2][x], gA[3][x])));
-        b.hiA[x] = __double2int_rd(fmax(fmax(gA[0][x], gA[1][x]), fmax(gA[2][x], gA[3][x])));
-        b.loB[x] = __double2int_rd(fmin(fmin(gB[0][x], gB[1][x]), fmin(gB[2][x], gB[3][x])));
-        b.hiB[x] = __double2int_rd(fmax(fmax(gB[0][x], gB[1][x]), fmax(gB[2][x], gB[3][x])));
-    }
-    const bool cellA = b.loA[0] == b.hiA[0] && b.loA[1] == b.hiA[1] && b.loA[2] == b.hiA[2];
-    const bool cellB = b.loB[0] == b.hiB[0] && b.loB[1] == b.hiB[1] && b.loB[2] == b.hiB[2];
-    b.actA = !cellA; b.actB = !cellB;
-    b.special = false; b.degenerate = false;
-    b.scell[0] = b.loA[0]; b.scell[1] = b.loA[1]; b.scell[2] = b.loA[2];
-    if (low_side) {
-        // degenerate first, as in the tet formulation (stage_a): its mass goes to the centroid cell
-        if (tet_det_sign(gA) == 0.0) {
-            b.degenerate = true;
-            b.actA = false;
-            if (weight_mode == 0) {
-                b.special = true;
-#pragma unroll
-                for (int x = 0; x < 3; ++x) b.scell[x] = __double2int_rd((gA[0][x] + gA[1][x] + gA[2][x] + gA[3][x]) / 4.0);
-            }
-        } else if (cellA) {
-            b.special = true;
-        }
-    }
-    // the face: vertices gA[fp[i]] (select chains: no dynamic register indexing)
-    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-    double fu[3], fv[3], fw[3];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int q = fp[i];
-        double c[3];
-#pragma unroll
-        for (int x = 0; x < 3; ++x) c[x] = q == 0 ? gA[0][x] : (q == 1 ? gA[1][x] : (q == 2 ? gA[2][x] : gA[3][x]));
-        fu[i] = ax == 0 ? c[0] : (ax == 1 ? c[1] : c[2]);
-        fv[i] = av == 0 ? c[0] : (av == 1 ? c[1] : c[2]);
-        fw[i] = aw == 0 ? c[0] : (aw == 1 ? c[1] : c[2]);
-    }
-    b.v0 = __double2int_rd(fmin(fmin(fv[0], fv[1]), fv[2]));
-    b.v1 = __double2int_ru(fmax(fmax(fv[0], fv[1]), fv[2])) - 1;
-    b.w0 = __double2int_rd(fmin(fmin(fw[0], fw[1]), fw[2]));
-    b.w1 = __double2int_ru(fmax(fmax(fw[0], fw[1]), fw[2])) - 1;
-    b.utop = __double2int_ru(fmax(fmax(fu[0], fu[1]), fu[2])) - 1;
-    const int la = ax == 0 ? b.loA[0] : (ax == 1 ? b.loA[1] : b.loA[2]);
-    const int lb = ax == 0 ? b.loB[0] : (ax == 1 ? b.loB[1] : b.loB[2]);
-    b.ulo = b.actA ? (b.actB ? min(la, lb) : la) : lb;
-    return b;
-}
-
-// the unit's particles: tet A and tet B in their own vertex order, unwrapped to the image of this
-// cell's corner 0, in grid units
-__device__ __forceinline__ void unit_tets(const Particles& p, const int i, const int j, const int k,
-                                          const unsigned long long uw, const double scale, double gA[4][3],
-                                          double gB[4][3]) {
-    double P0[3];
-    load_pos(p, corner_index(i, j, k, 0, p.N), P0);
-#pragma unroll
-    for (int v = 0; v < 4; ++v) {
-        double a[3], b[3];
-        load_pos(p, unit_particle(i, j, k, unit_nib(uw, 3 + v), p.N), a);
-        load_pos(p, unit_particle(i, j, k, unit_nib(uw, 7 + v), p.N), b);
-#pragma unroll
-        for (int x = 0; x < 3; ++x) {
-            // (corner 0 itself comes back unchanged: x - L * rint(0) = x)
-            gA[v][x] = __dmul_rn(unwrap1(a[x], P0[x], p.L, p.inv_L), scale);
-            gB[v][x] = __dmul_rn(unwrap1(b[x], P0[x], p.L, p.inv_L), scale);
-        }
-    }
-}
-
-// ---------------------------------------------------------------- census / scatter of the units
-// One thread per unit (12 per Lagrangian cell): the tiles where the unit has jobs -- the tiles
-// met by the face's column rectangle, from the lowest cell of its active tets up to the face's
-// top along the chord axis -- plus the tile of tet A's special.  SCATTER = false: counts per
-// (tile, class); true: the unit ids into the per-tile lists.  Uniform grids, every unit shorter
-// than G - 8 cells (one periodic image per tile; the host checks max_extent).
-// (One thread per cell with the 11 particles loaded once was measured too: 168 registers and 46
-// serial list entries per thread, 40 % slower than this.)
-constexpr int FCENSUS_THREADS = 128;
-template <bool SCATTER>
-__global__ void __launch_bounds__(FCENSUS_THREADS) k_face_census(Particles p, Space s, const int ax,
-                                                                 const int weight_mode, unsigned int* counts,
-                                                                 const unsigned long long* offsets,
-                                                                 unsigned int* cursors, unsigned int* pair_ids) {
-    const int N = p.N;
-    const int64_t nunit = (int64_t)N * N * N * FACE_UNITS;
-    const int64_t uid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (uid >= nunit) return;
-    const int64_t cell = uid / FACE_UNITS;
-    const int f = (int)(uid - cell * FACE_UNITS);
-    const int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((int64_t)N * N));
-    const unsigned long long uw = c_face_units[f];
-    double gA[4][3], gB[4][3];
-    unit_tets(p, i, j, k, uw, level_scale(s, 0), gA, gB);
-    const int fp[3] = {unit_nib(uw, 0), unit_nib(uw, 1), unit_nib(uw, 2)};
-    const UnitBox b = unit_box(gA, gB, fp, unit_low_side(uw), ax, weight_mode);
-    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-    const int nt = s.nt;
-    // tile box (unwrapped tile coordinates) of the jobs, per grid axis
-    int t0[3] = {0, 0, 0}, t1[3] = {-1, -1, -1};
-    if ((b.actA || b.actB) && b.v1 >= b.v0 && b.w1 >= b.w0 && b.utop >= b.ulo) {
-        const int u0 = floor_div(b.ulo, TILE), u1 = floor_div(b.utop, TILE);
-        const int v0 = floor_div(b.v0, TILE), v1 = floor_div(b.v1, TILE);
-        const int w0 = floor_div(b.w0, TILE), w1 = floor_div(b.w1, TILE);
-#pragma unroll
-        for (int x = 0; x < 3; ++x) {
-            t0[x] = x == ax ? u0 : (x == av ? v0 : w0);
-            t1[x] = x == ax ? u1 : (x == av ? v1 : w1);
-        }
-    }
-    auto emit = [&](const int tx, const int ty, const int tz, const int cls) {
-        const long long bin = (((long long)wrap_mod(tx, nt) * nt + wrap_mod(ty, nt)) * nt + wrap_mod(tz, nt)) * N_CLASSES + cls;
-        const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
-        const int leader = __ffs(peers) - 1;
-        if (!SCATTER) {
-            if ((int)(threadIdx.x & 31) == leader) atomicAdd(&counts[bin], (unsigned int)__popc(peers));
-        } else {
-            unsigned int base = 0;
-            if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&cursors[bin], (unsigned int)__popc(peers));
-            base = __shfl_sync(peers, base, leader);
-            pair_ids[offsets[bin] + base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u))] = (unsigned int)uid;
-        }
-    };
-    bool special_done = !b.special;
-    const int st[3] = {floor_div(b.scell[0], TILE), floor_div(b.scell[1], TILE), floor_div(b.scell[2], TILE)};
-    for (int tx = t0[0]; tx <= t1[0]; ++tx)
-        for (int ty = t0[1]; ty <= t1[1]; ++ty)
-            for (int tz = t0[2]; tz <= t1[2]; ++tz) {
-                // class: the face's columns inside this tile (large first in the work items)
-                const int tv = av == 0 ? tx : (av == 1 ? ty : tz), tw = aw == 0 ? tx : (aw == 1 ? ty : tz);
-                const int nv = min(b.v1, tv * TILE + TILE - 1) - max(b.v0, tv * TILE) + 1;
-                const int nw = min(b.w1, tw * TILE + TILE - 1) - max(b.w0, tw * TILE) + 1;
-                emit(tx, ty, tz, nv * nw > 4 ? 1 : 0);
-                if (b.special && tx == st[0] && ty == st[1] && tz == st[2]) special_done = true;
-            }
-    if (!special_done) emit(st[0], st[1], st[2], 0);
-}
-
-// ---------------------------------------------------------------- records of the (unit, tile) pairs
+// ---------------------------------------------------------------- the row word of one face
 // The row word of ONE face (face_rows in psd_kernels.cuh does a tet's four): first row in bits
 // 0..2, then 7 bits per row (first column, columns); returns the number of jobs.  pu / pv / pw:
 // the 3 vertices, tile-local; lou: lowest cell (along the chord axis) that can receive anything.
@@ -299,339 +114,10 @@ __device__ __forceinline__ int face_rows1(const double pu[3], const double pv[3]
     return c;
 }
 
-// Record of a (unit, tile) pair, 13 doubles (104 bytes), one after the other:
-//   [0..8]  the face's vertices, tile-local, (u, v, w) per vertex (u = chord axis)
-//   [9]     weight of tet A (6 m / det, or 1 in signed-volume mode) -- or the value of tet A's special
-//   [10]    weight of tet B
-//   [11]    the face's row word (u64)
-//   [12]    u64: bits 0..2 / 3..5 first / last cell of tet A along u in the tile, 6..8 / 9..11 of
-//           tet B (first > last: the tet adds nothing here), 12 special, 13..21 its cell, 22..28 jobs
-constexpr int FREC_DOUBLES = 13;
-constexpr int FREC_THREADS = 128;
-template <int ROWS>  // 0: rows in fp64, 1: in fp32
-__global__ void __launch_bounds__(FREC_THREADS, 6) k_face_records(DepositArgs A) {
-    constexpr int SS = 33;
-    __shared__ unsigned long long stg[FREC_THREADS / 32][FREC_DOUBLES * SS];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* sd = reinterpret_cast<double*>(stg[warp]);
-    const Item item = A.items[blockIdx.x];
-    int level, org[3];
-    double* out;
-    long long str[3];
-    tile_geometry(A.space, item.tile, level, org, out, str);
-    const int G = A.space.G, ax = A.chord_axis;
-    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-    const int N = A.part.N;
-    for (unsigned int k0 = 0; k0 < item.count; k0 += FREC_THREADS) {
-        const unsigned int kk = k0 + threadIdx.x;
-        __syncwarp();
-        if (kk < item.count) {
-            const unsigned int uid = A.pair_ids[item.begin + (item.count - 1u - kk)];
-            const unsigned int cell = uid / FACE_UNITS;
-            const int f = (int)(uid - cell * FACE_UNITS);
-            const int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((unsigned int)N * N));
-            const unsigned long long uw = c_face_units[f];
-            double gA[4][3], gB[4][3];
-            unit_tets(A.part, i, j, k, uw, level_scale(A.space, 0), gA, gB);
-            const int fp[3] = {unit_nib(uw, 0), unit_nib(uw, 1), unit_nib(uw, 2)};
-            const UnitBox b = unit_box(gA, gB, fp, unit_low_side(uw), ax, A.weight_mode);
-            int o[3];
-#pragma unroll
-            for (int x = 0; x < 3; ++x)  // the image of the tile that meets the unit
-                o[x] = org[x] - floor_div(org[x] + TILE - 1 - min(b.loA[x], b.loB[x]), G) * G;
-            const int ou = ax == 0 ? o[0] : (ax == 1 ? o[1] : o[2]);
-            const int ov = av == 0 ? o[0] : (av == 1 ? o[1] : o[2]);
-            const int ow = aw == 0 ? o[0] : (aw == 1 ? o[1] : o[2]);
-            // the face, tile-local, (u, v, w)
-            double pu[3], pv[3], pw[3];
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                const int t = fp[q];
-                double c[3];
-#pragma unroll
-                for (int x = 0; x < 3; ++x) c[x] = t == 0 ? gA[0][x] : (t == 1 ? gA[1][x] : (t == 2 ? gA[2][x] : gA[3][x]));
-                pu[q] = (ax == 0 ? c[0] : (ax == 1 ? c[1] : c[2])) - (double)ou;
-                pv[q] = (av == 0 ? c[0] : (av == 1 ? c[1] : c[2])) - (double)ov;
-                pw[q] = (aw == 0 ? c[0] : (aw == 1 ? c[1] : c[2])) - (double)ow;
-                sd[(3 * q + 0) * SS + lane] = pu[q];
-                sd[(3 * q + 1) * SS + lane] = pv[q];
-                sd[(3 * q + 2) * SS + lane] = pw[q];
-            }
-            // weights and ranges along u of the two tets
-            const double detA = tet_det(gA), detB = tet_det(gB);
-            double wA = A.weight_mode == 0 ? (detA != 0.0 ? 6.0 * A.mass_per_tet / detA : 0.0) : 1.0;
-            const double wB = A.weight_mode == 0 ? (detB != 0.0 ? 6.0 * A.mass_per_tet / detB : 0.0) : 1.0;
-            const int laU = ax == 0 ? b.loA[0] : (ax == 1 ? b.loA[1] : b.loA[2]), haU = ax == 0 ? b.hiA[0] : (ax == 1 ? b.hiA[1] : b.hiA[2]);
-            const int lbU = ax == 0 ? b.loB[0] : (ax == 1 ? b.loB[1] : b.loB[2]), hbU = ax == 0 ? b.hiB[0] : (ax == 1 ? b.hiB[1] : b.hiB[2]);
-            int cloA = max(laU - ou, 0), chiA = min(haU - ou, TILE - 1);
-            int cloB = max(lbU - ou, 0), chiB = min(hbU - ou, TILE - 1);
-            if (!b.actA || cloA > chiA) { cloA = TILE - 1; chiA = 0; }
-            if (!b.actB || cloB > chiB) { cloB = TILE - 1; chiB = 0; }
-            const bool anyA = cloA <= chiA, anyB = cloB <= chiB;
-            unsigned long long rows = 0ull;
-            int njobs = 0;
-            if (anyA || anyB) {
-                const int lou = anyA ? (anyB ? min(cloA, cloB) : cloA) : cloB;
-                njobs = ROWS ? face_rows1<float>(pu, pv, pw, lou, rows) : face_rows1<double>(pu, pv, pw, lou, rows);
-            }
-            // tet A's special, if its cell is in this tile
-            unsigned int special = 0u, scell = 0u;
-            if (b.special) {
-                const int c0 = b.scell[0] - o[0], c1 = b.scell[1] - o[1], c2 = b.scell[2] - o[2];
-                if ((unsigned)c0 < (unsigned)TILE && (unsigned)c1 < (unsigned)TILE && (unsigned)c2 < (unsigned)TILE) {
-                    special = 1u; scell = (unsigned int)((c0 * TILE + c1) * TILE + c2);
-                    wA = (A.weight_mode == 0 || b.degenerate) ? A.mass_per_tet : detA * (1.0 / 6.0);
-                }
-            }
-            sd[9 * SS + lane] = wA;
-            sd[10 * SS + lane] = wB;
-            stg[warp][11 * SS + lane] = rows;
-            stg[warp][12 * SS + lane] = (unsigned long long)((unsigned int)cloA | (unsigned int)chiA << 3 | (unsigned int)cloB << 6 |
-                                                             (unsigned int)chiB << 9 | special << 12 | scell << 13 |
-                                                             (unsigned int)njobs << 22);
-        }
-        __syncwarp();
-        const unsigned int kw = k0 + 32u * warp;
-        if (kw < item.count) {
-            const int valid = (int)min(32u, item.count - kw);
-            unsigned long long* dst = reinterpret_cast<unsigned long long*>(const_cast<double*>(A.rec_g)) +
-                                      ((long long)(item.begin - A.rec_pair_begin) + kw) * FREC_DOUBLES;
-#pragma unroll
-            for (int q = 0; q < FREC_DOUBLES; ++q) {
-                const int d = q * 32 + lane;
-                const int jr = (d * 5042) >> 16;  // d / 13 for d < 416
-                const int c = d - jr * FREC_DOUBLES;
-                if (jr < valid) dst[d] = stg[warp][c * SS + jr];
-            }
-        }
-    }
-}
-
-// ---------------------------------------------------------------- deposit of the face units
-__device__ __forceinline__ double frec_d(const DepositArgs& A, long long r, int c) { return __ldg(A.rec_g + r * FREC_DOUBLES + c); }
-__device__ __forceinline__ unsigned long long frec_u(const DepositArgs& A, long long r, int c) {
-    return __ldg(reinterpret_cast<const unsigned long long*>(A.rec_g) + r * FREC_DOUBLES + c);
-}
 // weight of a cell of the column: tet A's if the cell is in A's range, minus tet B's if in B's
 __device__ __forceinline__ double unit_weight(const double wA, const double wB, const unsigned int rng, const int c) {
     const int cloA = rng & 7, chiA = (rng >> 3) & 7, cloB = (rng >> 6) & 7, chiB = (rng >> 9) & 7;
     return ((c >= cloA) & (c <= chiA) ? wA : 0.0) - ((c >= cloB) & (c <= chiB) ? wB : 0.0);
-}
-
-// As k_deposit_tiles<COUNT, true>, with one face per slot and two tets per face; the tile is
-// flushed as 64-bit integers (the grid is in fixed point until k_fixed_to_double).
-constexpr int FDEP_MIN_CTAS = 6;
-template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, FDEP_MIN_CTAS) k_deposit_faces(DepositArgs A) {
-    extern __shared__ double smem[];
-    double* acc = smem;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* wpoly = smem + TILE_CELLS + warp * WARP_SCRATCH_REC;  // [3 * LB_SLOTS][32]
-    PolyBuf<32> poly{wpoly + lane};
-    poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; poly.at(7, 1) = 1.0; poly.at(7, 2) = 0.0;
-    poly.at(8, 1) = 1.0; poly.at(8, 2) = 1.0; poly.at(9, 1) = 0.0; poly.at(9, 2) = 1.0;
-    bool slot6_dirty = false;
-
-    const Item item = A.items[blockIdx.x];
-    int level, org[3];
-    double* out;
-    long long str[3];
-    tile_geometry(A.space, item.tile, level, org, out, str);
-    const int ax = A.chord_axis;
-    const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
-    const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1), sv = av == 0 ? 64 : (av == 1 ? 8 : 1), sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
-
-    __shared__ unsigned int sh_next;
-    for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) acc[i] = 0.0;
-    if (threadIdx.x == 0) sh_next = 0u;
-    __syncthreads();
-    JobCounters cnt = {0, 0, 0, 0, 0};
-
-    for (;;) {
-        unsigned int base = 0;
-        if (lane == 0) base = atomicAdd(&sh_next, 32u);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (base >= item.count) break;
-        const bool have = base + lane < item.count;
-        const long long rb = (long long)(item.begin - A.rec_pair_begin) + base;
-        int njobs = 0;
-        if (have) {
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(A.rec_g + (rb + lane) * FREC_DOUBLES));
-            const unsigned int word = (unsigned int)frec_u(A, rb + lane, 12);
-            njobs = (int)((word >> 22) & 127u);
-            if ((word >> 12) & 1u) tile_add(acc, (int)((word >> 13) & 511u), tile_share(frec_d(A, rb + lane, 9), A.acc_scale));
-        }
-        int pre = njobs;
-        for (int o = 1; o < 32; o <<= 1) {
-            int y = __shfl_up_sync(0xffffffffu, pre, o);
-            if (lane >= o) pre += y;
-        }
-        const int total = __shfl_sync(0xffffffffu, pre, 31);
-        pre -= njobs;
-#pragma unroll 1
-        for (int jb = 0; jb < total; jb += 32) {
-            const int job = jb + lane;
-            int slot = 0;
-#pragma unroll
-            for (int step = 16; step; step >>= 1) {
-                int probe = __shfl_sync(0xffffffffu, pre, slot + step);
-                if (probe <= job) slot += step;
-            }
-            const int spre = __shfl_sync(0xffffffffu, pre, slot);
-            const bool act = job < total;
-            unsigned int f_order = 0, f_info = 0, f_floors = 0, f_aux = 0;
-            int kpl = 0;
-            double f_wA = 0.0, f_wB = 0.0;
-            if (act) {
-                if (COUNT) cnt.jobs++;
-                const long long rs = rb + slot;
-                // (row, column) of the job from the face's row word
-                int local = job - spre;
-                unsigned long long rw = frec_u(A, rs, 11);
-                int cv = (int)(rw & 7ull);
-                rw >>= 3;
-#pragma unroll
-                for (int r = 0; r < TILE; ++r) {
-                    const int n = (int)(rw >> 3) & 15;
-                    if (local < n) break;
-                    local -= n; ++cv; rw >>= 7;
-                }
-                const int cw = ((int)rw & 7) + local;
-                const unsigned int word = (unsigned int)frec_u(A, rs, 12);
-                const unsigned int rng = word & 4095u;
-                const bool spc = (word >> 12) & 1u;
-                const int cloA = rng & 7, chiA = (rng >> 3) & 7, cloB = (rng >> 6) & 7, chiB = (rng >> 9) & 7;
-                const bool anyA = cloA <= chiA, anyB = cloB <= chiB;
-                const int c_lo = anyA ? (anyB ? min(cloA, cloB) : cloA) : cloB;
-                const int c_hi = anyA ? (anyB ? max(chiA, chiB) : chiA) : chiB;
-                const double ov = (double)cv, ow = (double)cw;
-                double U[3], V[3], W[3];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) {
-                    U[i] = frec_d(A, rs, 3 * i);
-                    V[i] = frec_d(A, rs, 3 * i + 1) - ov;
-                    W[i] = frec_d(A, rs, 3 * i + 2) - ow;
-                }
-                double wA = spc ? 0.0 : frec_d(A, rs, 9), wB = frec_d(A, rs, 10);
-                if (slot6_dirty) { poly.at(6, 1) = 0.0; poly.at(6, 2) = 0.0; slot6_dirty = false; }
-                const LBResult lb = tri_square_clip<32>(poly, U, V, W);
-                FaceClip fc;
-                if (lb.amb) {
-#pragma unroll
-                    for (int i = 0; i < 3; ++i) { poly.at(i, 0) = U[i]; poly.at(i, 1) = V[i]; poly.at(i, 2) = W[i]; }
-                    fc = face_clip_general(wpoly + lane);
-                    slot6_dirty = true;
-                    if (COUNT) cnt.general++;
-                } else {
-                    fc = poly_area_moment<32>(poly, lb.order, lb.n);
-                    if (lb.sign < 0) { wA = -wA; wB = -wB; }
-                }
-                if (fc.n >= 3 && fc.ice > c_lo) {
-                    if (COUNT) cnt.face_clips++;
-                    const FaceRun fr = face_run(fc, c_lo, c_hi);
-                    const int colofs = cv * sv + cw * sw;
-                    {
-                        const int full_hi = min(fr.t_hi, fc.ifl - 1);  // cells entirely below Q
-                        if (fc.A != 0.0) {
-#pragma unroll
-                            for (int cc = 0; cc < TILE; ++cc) {
-                                const int c = c_lo + cc;
-                                if (c > full_hi) break;
-                                const double wc = unit_weight(wA, wB, rng, c);
-                                if (wc != 0.0) {
-                                    tile_add(acc, colofs + c * su, tile_share(wc * fc.A, A.acc_scale));
-                                    if (COUNT) cnt.cells++;
-                                }
-                            }
-                        }
-                        if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {  // the cell holding umin
-                            const double D = fma(-(double)fc.ifl, fc.A, fc.M1) * unit_weight(wA, wB, rng, fc.ifl);
-                            if (D != 0.0) {
-                                tile_add(acc, colofs + fc.ifl * su, tile_share(D, A.acc_scale));
-                                if (COUNT) cnt.cells++;
-                            }
-                        }
-                    }
-                    kpl = max(fr.a_last - fr.a_first + 1, 0);
-                    f_order = fc.order;
-                    f_floors = fc.floors;
-                    f_aux = (unsigned)fr.a_first | rng << 4;
-                    f_info = (unsigned)colofs | (unsigned)c_lo << 11 | (unsigned)c_hi << 14 | (unsigned)fc.n << 17 | fc.below0 << 20;
-                    f_wA = wA; f_wB = wB;
-                }
-            }
-            __syncwarp();
-            // ---- the cutting planes of the 32 polygons, lane = plane
-            int pre2 = kpl;
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(0xffffffffu, pre2, o);
-                if (lane >= o) pre2 += y;
-            }
-            const int total2 = __shfl_sync(0xffffffffu, pre2, 31);
-            pre2 -= kpl;
-            for (int eb = 0; eb < total2; eb += 32) {
-                const int e = eb + lane;
-                int src = 0;
-#pragma unroll
-                for (int step = 16; step; step >>= 1) {
-                    int probe = __shfl_sync(0xffffffffu, pre2, src + step);
-                    if (probe <= e) src += step;
-                }
-                const int s_pre = __shfl_sync(0xffffffffu, pre2, src);
-                const unsigned int s_order = __shfl_sync(0xffffffffu, f_order, src);
-                const unsigned int s_info = __shfl_sync(0xffffffffu, f_info, src);
-                const unsigned int s_floors = __shfl_sync(0xffffffffu, f_floors, src);
-                const unsigned int s_aux = __shfl_sync(0xffffffffu, f_aux, src);
-                const double s_wA = __shfl_sync(0xffffffffu, f_wA, src);
-                const double s_wB = __shfl_sync(0xffffffffu, f_wB, src);
-                if (e < total2) {
-                    const int a = (int)(s_aux & 15u) + (e - s_pre);
-                    const unsigned int rng = s_aux >> 4;
-                    const int colofs = s_info & 511;
-                    const int c_lo = (s_info >> 11) & 7, c_hi = (s_info >> 14) & 7, n = (s_info >> 17) & 7;
-                    PolyBuf<32> qs{wpoly + src};
-                    const double R = plane_integral6_mask<32>(qs, s_order, n, (double)a, plane_mask_from_floors(s_floors, (s_info >> 20) & 127u, n, a)) * (1.0 / 6.0);
-                    if (COUNT) cnt.plane_evals++;
-                    if (R != 0.0) {
-                        if (a <= c_hi) {
-                            const double x = R * unit_weight(s_wA, s_wB, rng, a);
-                            if (x != 0.0) { tile_add(acc, colofs + a * su, tile_share(x, A.acc_scale)); if (COUNT) cnt.cells++; }
-                        }
-                        if (a - 1 >= c_lo) {
-                            const double x = -R * unit_weight(s_wA, s_wB, rng, a - 1);
-                            if (x != 0.0) { tile_add(acc, colofs + (a - 1) * su, tile_share(x, A.acc_scale)); if (COUNT) cnt.cells++; }
-                        }
-                    }
-                }
-            }
-            __syncwarp();
-        }
-    }
-    __syncthreads();
-    // ---- flush: 64-bit integer reductions (modulo 2^64), the grid is in fixed point for now
-    {
-        const unsigned int* a = reinterpret_cast<const unsigned int*>(acc);
-        unsigned long long* o64 = reinterpret_cast<unsigned long long*>(out);
-        for (int i = threadIdx.x; i < TILE_CELLS; i += DEP_THREADS) {
-            const unsigned long long v = ((unsigned long long)a[TILE_CELLS + i] << 32) | a[i];
-            if (v) {
-                int cz = i & 7, cy = (i >> 3) & 7, cx = i >> 6;
-                atomicAdd(o64 + cx * str[0] + cy * str[1] + cz, v);
-            }
-        }
-    }
-    if (COUNT) {
-        unsigned int a = __reduce_add_sync(0xffffffffu, cnt.jobs), b = __reduce_add_sync(0xffffffffu, cnt.face_clips);
-        unsigned int c = __reduce_add_sync(0xffffffffu, cnt.plane_evals), d = __reduce_add_sync(0xffffffffu, cnt.cells);
-        const unsigned int e = __reduce_add_sync(0xffffffffu, cnt.general);
-        if (lane == 0) {
-            atomicAdd(&A.stats[ST_TASKS], (unsigned long long)a);
-            atomicAdd(&A.stats[ST_FACE_CLIPS], (unsigned long long)b);
-            atomicAdd(&A.stats[ST_PLANE_CLIPS], (unsigned long long)c);
-            atomicAdd(&A.stats[ST_CELLS], (unsigned long long)d);
-            if (e) atomicAdd(&A.stats[ST_GENERAL], (unsigned long long)e);
-        }
-    }
 }
 
 // the grid from fixed point (two's complement, unit inv_scale) to fp64, in place
@@ -643,14 +129,7 @@ __global__ void __launch_bounds__(256) k_fixed_to_double(double* grid, const lon
     }
 }
 
-// ================================================================ shared faces on (tet, tile) pairs
-// The same sharing without a census of its own: the binning stays by (tet, tile) pair.  In the
-// pair (T, X) a face F of T, shared with the neighbour N, is clipped -- once, for both tets -- if
-// T owns F or if N does not meet tile X (then no pair (N, X) exists); it is skipped if N owns it
-// and the pair (N, X) exists, which clips it there.  Every decision is local to the pair: the
-// neighbours' far vertices are four more particles.  The chord axis is one per TILE (all pairs
-// that add to a column must agree on it): the axis that minimises the tile's column count,
-// chosen from the tet census (k_tile_axis), or one for the whole deposit.
+// ---------------------------------------------------------------- neighbours, per-tet table
 // per (tet t6, face f): bits 0..5 the neighbour's Lagrangian cell as offset + 1 (2 bits per axis),
 // 18 this tet owns the face (it is tet A of the face's unit), 19..21 the neighbour's t6
 __device__ __constant__ unsigned int c_tet_nbr[6][4] = {
@@ -708,7 +187,7 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
     long long str[3];
     tile_geometry(A.space, item.tile, level, org, out, str);
     const int G = A.space.G;
-    const int ax = A.tile_axis ? (int)A.tile_axis[item.tile] : A.chord_axis;
+    const int ax = A.chord_axis;
     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
     const int N = A.part.N;
     const double scale = level_scale(A.space, 0);
@@ -842,7 +321,7 @@ __device__ __forceinline__ unsigned long long rec2_u(const DepositArgs& A, long 
 // As k_deposit_tiles<COUNT, true> on the records of k_pair_records2: four faces per slot, each with
 // the weight and range of the neighbour behind it; the tile is flushed as 64-bit integers.
 template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, FDEP_MIN_CTAS) k_deposit_tiles2(DepositArgs A) {
+__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS_REC) k_deposit_tiles2(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -857,7 +336,7 @@ __global__ void __launch_bounds__(DEP_THREADS, FDEP_MIN_CTAS) k_deposit_tiles2(D
     double* out;
     long long str[3];
     tile_geometry(A.space, item.tile, level, org, out, str);
-    const int ax = A.tile_axis ? (int)A.tile_axis[item.tile] : A.chord_axis;
+    const int ax = A.chord_axis;
     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
     const int su = ax == 0 ? 64 : (ax == 1 ? 8 : 1), sv = av == 0 ? 64 : (av == 1 ? 8 : 1), sw = aw == 0 ? 64 : (aw == 1 ? 8 : 1);
 

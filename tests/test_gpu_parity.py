@@ -381,6 +381,7 @@ def test_fp32_rows_cover_the_fp64_rows(psd, ctx, oracle, case):
     else:                          # tets far smaller than a cell: slopes of every size inside one column
         pos, G = crossing_field(16, 0.5), 64
     ora, _ = oracle.deposit_uniform(pos, 1.0, 1.0, G)
+    ctx.psd_set_option(psd.OPT_FACE_SHARING, 0)  # the tet formulation: its record kernel holds the check
     ctx.psd_set_option(psd.OPT_COUNTERS, 1)
     ctx.psd_set_option(psd.OPT_CHUNK, 256)
     res = {}
@@ -401,11 +402,11 @@ def test_fp32_rows_cover_the_fp64_rows(psd, ctx, oracle, case):
 @pytest.mark.parametrize("axis", [0, 1, 2])
 @pytest.mark.parametrize("case", ["crossing", "crossing_f64", "lattice", "jittered", "coincident", "box_mass"])
 def test_shared_face_path_parity(psd, ctx, oracle, case, axis):
-    """PSD_OPT_FACE_SHARING: every face of the tessellation clipped once for its two tets (units =
-    the 12 faces a Lagrangian cell owns, one chord axis per deposit, 64-bit fixed-point tiles and
-    grid).  Against the oracle: crossing fields (inverted tets), the exact lattice (every decision a
-    tie: the general clip), the paper's jittered lattice on a coarse grid (most tets inside one cell:
-    the units' specials), coincident particles (degenerate tets), L != 1 and M != 1."""
+    """PSD_OPT_FACE_SHARING: every face of the tessellation clipped once for its two tets (in the
+    pair of the tet that owns it, one chord axis per deposit, 64-bit fixed-point tiles and grid).
+    Against the oracle: crossing fields (inverted tets), the exact lattice (every decision a tie: the
+    general clip), the paper's jittered lattice on a coarse grid (most tets inside one cell: the
+    pairs' specials), coincident particles (degenerate tets), L != 1 and M != 1."""
     import torch
     L, M = 1.0, 1.0
     if case == "crossing":
@@ -427,10 +428,20 @@ def test_shared_face_path_parity(psd, ctx, oracle, case, axis):
     ctx.psd_build_tets(to_dev(pos), L, M)
     g = ctx.psd_deposit_uniform(G)
     s = ctx.psd_get_stats()
-    assert s.n_unit_pairs > 0, "the shared-face path did not run"
+    assert s.shared_faces == 1, "the shared-face path did not run"
     assert s.n_pairs > 0 and s.n_degenerate == st["n_degenerate"]  # the tet census still runs
     assert_mass(g.sum(), M)
     assert_parity(g.cpu().numpy(), ora, what=f"{case}, axis {axis}")
+    # the face jobs found in fp64 (PSD_OPT_ROWS_FP32 = 0): no more jobs, the same deposit
+    ctx.psd_set_option(psd.OPT_ROWS_FP32, 0)
+    ctx.psd_build_tets(to_dev(pos), L, M)
+    g64 = ctx.psd_deposit_uniform(G)
+    s64 = ctx.psd_get_stats()
+    assert s64.shared_faces == 1 and s64.n_face_jobs <= s.n_face_jobs
+    # (on the exact lattice the margin adds jobs whose polygon is a segment on a lattice line)
+    assert s64.n_face_clips == s.n_face_clips or case == "lattice"
+    assert float((g - g64).abs().max()) <= 1e-13 * float(g64.max())
+    ctx.psd_set_option(psd.OPT_ROWS_FP32, 1)
     if case == "crossing":
         # fewer jobs than the tet formulation with the same axis (each face once), same deposit
         ctx.psd_set_option(psd.OPT_FACE_SHARING, 0)
@@ -438,7 +449,7 @@ def test_shared_face_path_parity(psd, ctx, oracle, case, axis):
         ctx.psd_build_tets(to_dev(pos), L, M)
         g0 = ctx.psd_deposit_uniform(G)
         s0 = ctx.psd_get_stats()
-        assert s0.n_unit_pairs == 0 and 0.45 * s0.n_face_jobs < s.n_face_jobs < 0.62 * s0.n_face_jobs
+        assert s0.shared_faces == 0 and 0.45 * s0.n_face_jobs < s.n_face_jobs < 0.62 * s0.n_face_jobs
         assert float((g - g0).abs().max()) <= 1e-11 * float(g0.max())
         # signed-volume mode: every cell 1; the host-output call (grid converted slab by slab); and
         # accumulate = 1, which the fixed-point grid cannot serve (the tet formulation runs)
@@ -447,16 +458,16 @@ def test_shared_face_path_parity(psd, ctx, oracle, case, axis):
         ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
         ctx.psd_build_tets(to_dev(pos))
         gv = ctx.psd_deposit_uniform(G)
-        assert ctx.psd_get_stats().n_unit_pairs > 0
+        assert ctx.psd_get_stats().shared_faces == 1
         assert float((gv - 1.0).abs().max()) <= 1e-9
         ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 0)
         hg = torch.full((G, G, G), -1.0, dtype=torch.float64).pin_memory()
         ctx.psd_deposit_uniform_host(torch.from_numpy(pos).pin_memory(), G, hg)
-        assert ctx.psd_get_stats().n_unit_pairs > 0
+        assert ctx.psd_get_stats().shared_faces == 1
         assert_parity(hg.numpy(), ora, what="shared faces, host output")
         ctx.psd_build_tets(to_dev(pos))
         ctx.psd_deposit_uniform(G, g, accumulate=True)
-        assert ctx.psd_get_stats().n_unit_pairs == 0
+        assert ctx.psd_get_stats().shared_faces == 0
         assert_parity(g.cpu().numpy(), 2.0 * ora, what="shared faces, accumulate")
 
 
