@@ -320,8 +320,11 @@ __device__ __forceinline__ unsigned long long rec2_u(const DepositArgs& A, long 
 }
 // As k_deposit_tiles<COUNT, true> on the records of k_pair_records2: four faces per slot, each with
 // the weight and range of the neighbour behind it; the tile is flushed as 64-bit integers.
+#ifndef DEP2_MIN_CTAS
+#define DEP2_MIN_CTAS 6
+#endif
 template <bool COUNT>
-__global__ void __launch_bounds__(DEP_THREADS, DEP_MIN_CTAS_REC) k_deposit_tiles2(DepositArgs A) {
+__global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(DepositArgs A) {
     extern __shared__ double smem[];
     double* acc = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
