@@ -183,7 +183,8 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     // Uniform grids, not accumulating (the grid is in fixed point until the end), two tets plus a
     // tile shorter than the grid (one periodic image per pair, neighbours' ranges unambiguous).
     const bool pair_share = ctx->face_sharing && ctx->use_records && !space.patch_mode && !ctx->accumulate_now &&
-                            n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G;
+                            n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G &&
+                            (long long)max_extent <= TETINFO_MAX_EXTENT;
     const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_sharing - 1;
     ctx->last.shared_faces = pair_share ? 1 : 0;
     if (n_pairs > 0) {
@@ -229,8 +230,8 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.acc_inv_scale = std::ldexp(1.0, -(62 - eb));
             // what a pair needs of its tet and the four neighbours: determinant, cell range
             CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell)));
-            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)space.G / space.L,
-                                                                                ctx->tet_info.as<TetInfo>());
+            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)space.G / space.L, A.mass_per_tet,
+                                                                                ctx->weight_mode, ctx->tet_info.as<TetInfo>());
             ctx->launches += 1;
             A.tet_info = ctx->tet_info.p;
         }

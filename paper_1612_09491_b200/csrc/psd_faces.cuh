@@ -142,14 +142,22 @@ __device__ __constant__ unsigned int c_tet_nbr[6][4] = {
 };
 
 // Per tet, written once per deposit (k_tet_info) and read by the record kernel for the tet itself
-// and for its four neighbours: determinant (compensated, the tet's own vertex order -- one number
-// per tet wherever it is used), cell range in the image of its own corner 0.
+// and for its four neighbours (one 16-byte load each): the tet's weight 6 m / det (0 when det = 0;
+// det from the compensated determinant in the tet's own vertex order -- one number per tet wherever
+// it is used; in signed-volume mode the field holds det itself), and its cell range in the image
+// of its own corner 0: lo + 1024 in 12 bits per axis (bits 0..35; lo > -1024 and < 3072 for G <=
+// 2048 and ranges shorter than 512), hi - lo in 9 bits per axis (36..62), bit 63: det = 0.
 struct TetInfo {
-    double det;
-    int lo[3];
-    unsigned int ext;  // hi - lo per axis, 10 bits each (clamped: the shared-face path needs short tets anyway)
+    double val;
+    unsigned long long box;
 };
-__global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scale, TetInfo* info) {
+constexpr int TETINFO_MAX_EXTENT = 511;  // the host runs the tet formulation beyond
+__device__ __forceinline__ int tetinfo_lo(const TetInfo& e, int x) { return (int)((e.box >> (12 * x)) & 4095ull) - 1024; }
+__device__ __forceinline__ int tetinfo_ext(const TetInfo& e, int x) { return (int)((e.box >> (36 + 9 * x)) & 511ull); }
+__device__ __forceinline__ bool tetinfo_one_cell(const TetInfo& e) { return ((e.box >> 36) & 0x7ffffffull) == 0ull; }
+__device__ __forceinline__ bool tetinfo_degenerate(const TetInfo& e) { return (e.box >> 63) != 0ull; }
+__global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scale, const double mass_per_tet,
+                                                  const int weight_mode, TetInfo* info) {
     const int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
     const int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (id >= ntet) return;
@@ -157,12 +165,21 @@ __global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scal
     load_tet_vertices(p, id / 6, (int)(id % 6), P);
     Tet t;
     finish_tet(P, scale, t);
+    const double det = tet_det(t.g);
     TetInfo e;
-    e.det = tet_det(t.g);
-    e.lo[0] = t.lo[0]; e.lo[1] = t.lo[1]; e.lo[2] = t.lo[2];
-    e.ext = (unsigned int)min(t.hi[0] - t.lo[0], 1023) | (unsigned int)min(t.hi[1] - t.lo[1], 1023) << 10 |
-            (unsigned int)min(t.hi[2] - t.lo[2], 1023) << 20;
-    info[id] = e;
+    e.val = weight_mode == 0 ? (det != 0.0 ? 6.0 * mass_per_tet / det : 0.0) : det;
+    e.box = (unsigned long long)(det == 0.0) << 63;
+#pragma unroll
+    for (int x = 0; x < 3; ++x)
+        e.box |= (unsigned long long)((t.lo[x] + 1024) & 4095) << (12 * x) |
+                 (unsigned long long)min(t.hi[x] - t.lo[x], TETINFO_MAX_EXTENT) << (36 + 9 * x);
+    reinterpret_cast<double2*>(info)[id] = make_double2(e.val, __longlong_as_double((long long)e.box));
+}
+__device__ __forceinline__ TetInfo tetinfo_load(const TetInfo* info, int64_t id) {
+    const double2 v = __ldg(reinterpret_cast<const double2*>(info) + id);
+    TetInfo e;
+    e.val = v.x; e.box = (unsigned long long)__double_as_longlong(v.y);
+    return e;
 }
 
 // Record of a (tet, tile) pair, 23 doubles (184 bytes):
@@ -200,24 +217,23 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
             const int t6 = (int)(id - cell * 6u);
             const int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((unsigned int)N * N));
             const TetInfo* info = reinterpret_cast<const TetInfo*>(A.tet_info);
-            const TetInfo me = info[id];
+            const TetInfo me = tetinfo_load(info, (int64_t)id);
             double P[4][3];
             load_tet_vertices(A.part, (int64_t)cell, t6, P);
             int lo[3], hi[3], o[3];
 #pragma unroll
             for (int x = 0; x < 3; ++x) {
-                lo[x] = me.lo[x];
-                hi[x] = lo[x] + (int)((me.ext >> (10 * x)) & 1023u);
+                lo[x] = tetinfo_lo(me, x);
+                hi[x] = lo[x] + tetinfo_ext(me, x);
                 o[x] = org[x] - floor_div(org[x] + TILE - 1 - lo[x], G) * G;  // the image of the tile the tet meets
 #pragma unroll
                 for (int v = 0; v < 4; ++v) sd[(3 * v + x) * SS + lane] = __dmul_rn(P[v][x], scale) - (double)o[x];
             }
-            const double det = me.det;
-            const bool cellT = me.ext == 0u;
-            double wT = A.weight_mode == 0 ? (det != 0.0 ? 6.0 * A.mass_per_tet / det : 0.0) : 1.0;
+            const bool cellT = tetinfo_one_cell(me);
+            double wT = A.weight_mode == 0 ? me.val : 1.0;
             bool actT = true;
             unsigned int special = 0u, scell = 0u;
-            if (det == 0.0) {  // degenerate: whole mass to the centroid cell (Q6)
+            if (tetinfo_degenerate(me)) {  // degenerate: whole mass to the centroid cell (Q6)
                 actT = false;
                 if (A.weight_mode == 0) {
                     int c[3];
@@ -234,7 +250,7 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
                 actT = false;
                 special = 1u;
                 scell = (unsigned int)(((lo[0] - o[0]) * TILE + (lo[1] - o[1])) * TILE + (lo[2] - o[2]));
-                wT = A.weight_mode == 0 ? A.mass_per_tet : det * (1.0 / 6.0);
+                wT = A.weight_mode == 0 ? A.mass_per_tet : me.val * (1.0 / 6.0);
             }
             const int loU = ax == 0 ? lo[0] : (ax == 1 ? lo[1] : lo[2]), hiU = ax == 0 ? hi[0] : (ax == 1 ? hi[1] : hi[2]);
             const int oU = ax == 0 ? o[0] : (ax == 1 ? o[1] : o[2]);
@@ -251,24 +267,24 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
                 ni = ni < 0 ? ni + N : (ni >= N ? ni - N : ni);
                 nj = nj < 0 ? nj + N : (nj >= N ? nj - N : nj);
                 nk = nk < 0 ? nk + N : (nk >= N ? nk - N : nk);
-                const TetInfo en = info[(((int64_t)ni * N + nj) * N + nk) * 6 + (int)((nb >> 19) & 7u)];
+                const TetInfo en = tetinfo_load(info, (((int64_t)ni * N + nj) * N + nk) * 6 + (int)((nb >> 19) & 7u));
                 int nlo[3], nhi[3];
                 bool meets = true;
 #pragma unroll
                 for (int x = 0; x < 3; ++x) {
-                    int l = en.lo[x];
+                    int l = tetinfo_lo(en, x);
                     const int d = lo[x] - l;      // the two tets share a face: their ranges are close
                     l += 2 * d > G ? G : (2 * d < -G ? -G : 0);
                     nlo[x] = l - o[x];
-                    nhi[x] = nlo[x] + (int)((en.ext >> (10 * x)) & 1023u);
+                    nhi[x] = nlo[x] + tetinfo_ext(en, x);
                     meets = meets && nlo[x] <= TILE - 1 && nhi[x] >= 0;
                 }
-                const bool cellN = en.ext == 0u;
+                const bool cellN = tetinfo_one_cell(en);
                 const bool own = (nb >> 18) & 1u;
                 double wN = 0.0;
                 int cloN = TILE - 1, chiN = 0;
                 if (meets && !cellN) {
-                    wN = A.weight_mode == 0 ? (en.det != 0.0 ? 6.0 * A.mass_per_tet / en.det : 0.0) : 1.0;
+                    wN = A.weight_mode == 0 ? en.val : 1.0;
                     const int nl = ax == 0 ? nlo[0] : (ax == 1 ? nlo[1] : nlo[2]), nh = ax == 0 ? nhi[0] : (ax == 1 ? nhi[1] : nhi[2]);
                     cloN = max(nl, 0); chiN = min(nh, TILE - 1);
                     if (wN == 0.0) { cloN = TILE - 1; chiN = 0; }
