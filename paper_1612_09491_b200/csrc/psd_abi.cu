@@ -17,6 +17,10 @@
 
 using namespace psd;
 
+#ifndef PSD_CENSUS_CB
+#define PSD_CENSUS_CB 256  // threads per CTA of the census and scatter kernels
+#endif
+
 namespace {
 
 struct DevBuf {
@@ -128,7 +132,7 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     if (rc) return rc;
 
     CK(cudaEventRecord(ctx->ev[0], st));
-    const int cb = 256;
+    const int cb = PSD_CENSUS_CB;
     const unsigned int cgrid = (unsigned int)((ncell + cb - 1) / cb);
     k_census<false><<<cgrid, cb, 0, st>>>(ctx->part, space, ctx->tile_counts.as<unsigned int>(), nullptr,
                                           nullptr, nullptr, ctx->stats.as<unsigned long long>(),
@@ -1063,7 +1067,7 @@ int psd_deposit_uniform_static(int device, void* cuda_stream, const void* pos_de
     SCK(cudaMemsetAsync(sc, 0, offsetof(StaticScratch, totals), st));
     SCK(cudaMemsetAsync(grid_dev, 0, sizeof(double) * (size_t)G * G * G, st));
     k_validate<<<1184, 256, 0, st>>>(part, sc->stats);
-    const int cb = 256;
+    const int cb = PSD_CENSUS_CB;
     const unsigned int cgrid = (unsigned int)((ncell + cb - 1) / cb);
     k_census<false><<<cgrid, cb, 0, st>>>(part, space, sc->tile_counts, nullptr, nullptr, nullptr, sc->stats, sc->hist);
     k_scan_partials<<<nparts, SCAN_BLOCK, 0, st>>>(sc->tile_counts, n_bins, STATIC_CHUNK, sc->part_pairs, sc->part_items);
