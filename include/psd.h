@@ -65,7 +65,8 @@ enum {
     PSD_OPT_COUNTERS = 2,    /* 1: also count face jobs / non-empty clips / plane integrals / cell
                                 shares written during deposits (slower; for the work model).    */
     PSD_OPT_CHUNK = 3,       /* (tet,tile) pairs per work item of the binned path (default 2048) */
-    PSD_OPT_CHORD_AXIS = 4,  /* -1 (default): per-tet longest AABB axis; 0/1/2: fixed x/y/z      */
+    PSD_OPT_CHORD_AXIS = 4,  /* -1 (default): per-tet longest AABB axis in the tet formulation,
+                                the axis of PSD_OPT_FACE_SHARING with shared faces; 0/1/2: fixed x/y/z */
     PSD_OPT_REFINE_SUBBLOCK = 5 /* census used by psd_refine_patches.  0 (default): every tet is
                                 counted.  B in 1..64: the paper's memory-lean
                                 estimate (B = 8 there): the Lagrangian grid is
@@ -93,15 +94,16 @@ enum {
                                 margin of 1e-9 (0).  Either set holds every column with a non-empty
                                 polygon and the clip itself is fp64, so the deposit is the same;
                                 fp32 admits a few more empty jobs (n_face_jobs).               */
-    PSD_OPT_FACE_SHARING = 10, /* binned path, uniform grids.  1..3 (default 1): every face of the
-                                tessellation is clipped ONCE, for the two tets that share it, in
-                                the (tet, tile) pair of the tet that owns it; one chord axis for
-                                the whole deposit (value - 1 = x / y / z, unless
+    PSD_OPT_FACE_SHARING = 10, /* binned path (uniform grids and patches).  1..3 (default 1): every
+                                face of the tessellation is clipped ONCE, for the two tets that
+                                share it, in the (tet, tile) pair of the tet that owns it; one chord
+                                axis for the whole deposit (value - 1 = x / y / z, unless
                                 PSD_OPT_CHORD_AXIS fixes one); tiles and grid are summed in 64-bit
                                 fixed point (unit 2^-62 of the total mass) and converted to fp64 at
                                 the end.  Runs when twice the largest cell range of a tet plus a
-                                tile fits the grid, with pair records and accumulate = 0; else,
-                                and with 0, the tet formulation runs (stats.shared_faces).     */
+                                tile fits the grid (on every level), with pair records and
+                                accumulate = 0; else, and with 0, the tet formulation runs
+                                (stats.shared_faces).                                          */
     PSD_OPT_PATCH_RESTRICT = 7  /* psd_deposit_patches, PAPER.md:193 (coarser representations of the
                                 internal nodes).  1 (default): a listed patch whose 8 children are
                                 all listed too is not deposited into; it is filled afterwards by

@@ -184,11 +184,15 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     ctx->last.n_tiles = n_tiles;
     CK(cudaEventRecord(ctx->ev[2], st));
     // Shared faces (psd_faces.cuh): every face of the tessellation clipped once for its two tets.
-    // Uniform grids, not accumulating (the grid is in fixed point until the end), two tets plus a
-    // tile shorter than the grid (one periodic image per pair, neighbours' ranges unambiguous).
-    const bool pair_share = ctx->face_sharing && ctx->use_records && !space.patch_mode && !ctx->accumulate_now &&
-                            n_pairs > 0 && 2ll * (long long)max_extent + 2 + TILE < (long long)space.G &&
-                            (long long)max_extent <= TETINFO_MAX_EXTENT;
+    // Not accumulating (the grid is in fixed point until the end), two tets plus a tile shorter
+    // than the grid (one periodic image per pair, neighbours' ranges unambiguous), on every level:
+    // a range of e cells on level 0 is at most (e + 1) 2^l - 1 cells on level l.
+    const int top_level = space.patch_mode ? space.n_levels - 1 : 0;
+    const long long g0 = space.patch_mode ? space.base_G : space.G;
+    const long long ext_top = (((long long)max_extent + 1) << top_level);
+    const bool pair_share = ctx->face_sharing && ctx->use_records && !ctx->accumulate_now && n_pairs > 0 &&
+                            2ll * (long long)max_extent + 2 + TILE < g0 && 2ll * ext_top + 2 + TILE < (g0 << top_level) &&
+                            ext_top <= TETINFO_MAX_EXTENT && (g0 << top_level) <= 2048;
     const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_sharing - 1;
     ctx->last.shared_faces = pair_share ? 1 : 0;
     if (n_pairs > 0) {
@@ -233,10 +237,13 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             A.acc_scale = std::ldexp(1.0, 62 - eb);
             A.acc_inv_scale = std::ldexp(1.0, -(62 - eb));
             // what a pair needs of its tet and the four neighbours: determinant, cell range
-            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell)));
-            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)space.G / space.L, A.mass_per_tet,
-                                                                                ctx->weight_mode, ctx->tet_info.as<TetInfo>());
-            ctx->launches += 1;
+            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)));
+            for (int l = 0; l <= top_level; ++l) {
+                k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
+                    ctx->part, (double)(g0 << l) / space.L, A.mass_per_tet, ctx->weight_mode,
+                    ctx->tet_info.as<TetInfo>() + (size_t)l * (size_t)(6 * ncell));
+                ctx->launches += 1;
+            }
             A.tet_info = ctx->tet_info.p;
         }
         const size_t rec_bytes = pair_share ? sizeof(double) * REC2_DOUBLES : REC_BYTES;
@@ -352,8 +359,8 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
                                    cudaMemcpyDeviceToHost, ctx->copy_stream));
             }
         }
-        if (pair_share && n_slabs <= 1) {
-            k_fixed_to_double<<<1184, 256, 0, st>>>(space.out, (long long)space.G * space.G * space.G, A.acc_inv_scale);
+        if (pair_share && n_slabs <= 1) {  // all cells of the grid, or of the patches
+            k_fixed_to_double<<<1184, 256, 0, st>>>(space.out, n_tiles * (long long)TILE_CELLS, A.acc_inv_scale);
             ctx->launches += 1;
         }
         if (n_slabs > 1) {
@@ -635,6 +642,7 @@ int psd_deposit_patches(psd_ctx* ctx, const psd_patch* patches_host, int64_t n_p
     s.lookup = ctx->lookup.as<int>();
     s.patches = ctx->patches.as<PatchDev>();
     if (!accumulate) CK(cudaMemsetAsync(mass_dev, 0, sizeof(double) * (size_t)n_patch * P * P * P, ctx->stream));
+    ctx->accumulate_now = accumulate != 0;
     const int64_t nf = ctx->last.n_nonfinite;
     std::memset(&ctx->last, 0, sizeof(ctx->last));
     ctx->last.n_tets = 6ll * ctx->part.N * ctx->part.N * ctx->part.N;

@@ -114,10 +114,13 @@ __device__ __forceinline__ int face_rows1(const double pu[3], const double pv[3]
     return c;
 }
 
-// weight of a cell of the column: tet A's if the cell is in A's range, minus tet B's if in B's
-__device__ __forceinline__ double unit_weight(const double wA, const double wB, const unsigned int rng, const int c) {
-    const int cloA = rng & 7, chiA = (rng >> 3) & 7, cloB = (rng >> 6) & 7, chiB = (rng >> 9) & 7;
-    return ((c >= cloA) & (c <= chiA) ? wA : 0.0) - ((c >= cloB) & (c <= chiB) ? wB : 0.0);
+// weight of a cell of the column: tet A's if the cell is in A's range, minus tet B's if in B's.
+// cells: bit c = cell c is in A's range, bit 8 + c = in B's (range_mask)
+__device__ __forceinline__ unsigned int range_mask(const int clo, const int chi) {  // clo > chi: none
+    return clo <= chi ? ((2u << chi) - (1u << clo)) : 0u;
+}
+__device__ __forceinline__ double unit_weight(const double wA, const double wB, const unsigned int cells, const int c) {
+    return ((cells >> c) & 1u ? wA : 0.0) - ((cells >> (c + 8)) & 1u ? wB : 0.0);
 }
 
 // the grid from fixed point (two's complement, unit inv_scale) to fp64, in place
@@ -203,11 +206,13 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
     double* out;
     long long str[3];
     tile_geometry(A.space, item.tile, level, org, out, str);
-    const int G = A.space.G;
+    const int G = level_G(A.space, level);
     const int ax = A.chord_axis;
     const int av = ax == 2 ? 0 : ax + 1, aw = ax == 0 ? 2 : ax - 1;
     const int N = A.part.N;
-    const double scale = level_scale(A.space, 0);
+    const double scale = level_scale(A.space, level);
+    // the per-tet table of this tile's level (patch mode: one table per level, cell ranges differ)
+    const TetInfo* info = reinterpret_cast<const TetInfo*>(A.tet_info) + (long long)level * 6 * N * N * N;
     for (unsigned int k0 = 0; k0 < item.count; k0 += REC2_THREADS) {
         const unsigned int kk = k0 + threadIdx.x;
         __syncwarp();
@@ -216,7 +221,6 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
             const unsigned int cell = id / 6u;
             const int t6 = (int)(id - cell * 6u);
             const int k = (int)(cell % N), j = (int)((cell / N) % N), i = (int)(cell / ((unsigned int)N * N));
-            const TetInfo* info = reinterpret_cast<const TetInfo*>(A.tet_info);
             const TetInfo me = tetinfo_load(info, (int64_t)id);
             double P[4][3];
             load_tet_vertices(A.part, (int64_t)cell, t6, P);
@@ -430,6 +434,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                 const unsigned int rng = (unsigned int)((word >> 12) & 63ull) | (unsigned int)((word >> (18 + 6 * f)) & 63ull) << 6;
                 const bool spc = (word >> 2) & 1ull;
                 const int cloA = rng & 7, chiA = (rng >> 3) & 7, cloB = (rng >> 6) & 7, chiB = (rng >> 9) & 7;
+                const unsigned int cells = range_mask(cloA, chiA) | range_mask(cloB, chiB) << 8;
                 const bool anyA = cloA <= chiA, anyB = cloB <= chiB;
                 const int c_lo = anyA ? (anyB ? min(cloA, cloB) : cloA) : cloB;
                 const int c_hi = anyA ? (anyB ? max(chiA, chiB) : chiA) : chiB;
@@ -469,7 +474,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                             for (int cc = 0; cc < TILE; ++cc) {
                                 const int c = c_lo + cc;
                                 if (c > full_hi) break;
-                                const double wc = unit_weight(wA, wB, rng, c);
+                                const double wc = unit_weight(wA, wB, cells, c);
                                 if (wc != 0.0) {
                                     tile_add(acc, colofs + c * su, tile_share(wc * fc.A, A.acc_scale));
                                     if (COUNT) cnt.cells++;
@@ -477,7 +482,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                             }
                         }
                         if (fr.t_hi >= fc.ifl && fc.ifl >= c_lo) {  // the cell holding umin
-                            const double D = fma(-(double)fc.ifl, fc.A, fc.M1) * unit_weight(wA, wB, rng, fc.ifl);
+                            const double D = fma(-(double)fc.ifl, fc.A, fc.M1) * unit_weight(wA, wB, cells, fc.ifl);
                             if (D != 0.0) {
                                 tile_add(acc, colofs + fc.ifl * su, tile_share(D, A.acc_scale));
                                 if (COUNT) cnt.cells++;
@@ -487,7 +492,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                     kpl = max(fr.a_last - fr.a_first + 1, 0);
                     f_order = fc.order;
                     f_floors = fc.floors;
-                    f_aux = (unsigned)fr.a_first | rng << 4;
+                    f_aux = (unsigned)fr.a_first | cells << 4;
                     f_info = (unsigned)colofs | (unsigned)c_lo << 11 | (unsigned)c_hi << 14 | (unsigned)fc.n << 17 | fc.below0 << 20;
                     f_wA = wA; f_wB = wB;
                 }
@@ -518,7 +523,7 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                 const double s_wB = __shfl_sync(0xffffffffu, f_wB, src);
                 if (e < total2) {
                     const int a = (int)(s_aux & 15u) + (e - s_pre);
-                    const unsigned int rng = s_aux >> 4;
+                    const unsigned int cells = s_aux >> 4;
                     const int colofs = s_info & 511;
                     const int c_lo = (s_info >> 11) & 7, c_hi = (s_info >> 14) & 7, n = (s_info >> 17) & 7;
                     PolyBuf<32> qs{wpoly + src};
@@ -526,11 +531,11 @@ __global__ void __launch_bounds__(DEP_THREADS, DEP2_MIN_CTAS) k_deposit_tiles2(D
                     if (COUNT) cnt.plane_evals++;
                     if (R != 0.0) {
                         if (a <= c_hi) {
-                            const double x = R * unit_weight(s_wA, s_wB, rng, a);
+                            const double x = R * unit_weight(s_wA, s_wB, cells, a);
                             if (x != 0.0) { tile_add(acc, colofs + a * su, tile_share(x, A.acc_scale)); if (COUNT) cnt.cells++; }
                         }
                         if (a - 1 >= c_lo) {
-                            const double x = -R * unit_weight(s_wA, s_wB, rng, a - 1);
+                            const double x = -R * unit_weight(s_wA, s_wB, cells, a - 1);
                             if (x != 0.0) { tile_add(acc, colofs + (a - 1) * su, tile_share(x, A.acc_scale)); if (COUNT) cnt.cells++; }
                         }
                     }

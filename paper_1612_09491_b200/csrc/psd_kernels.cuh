@@ -419,7 +419,7 @@ struct DepositArgs {
     // rec_g == nullptr: the deposit kernel runs stage A itself (fused mode)
     const double* rec_g;
     unsigned long long rec_pair_begin;  // first pair (position in pair_ids) of the record buffer
-    const void* tet_info;               // shared faces (psd_faces.cuh): the per-tet table, TetInfo[6 N^3]
+    const void* tet_info;               // shared faces (psd_faces.cuh): the per-tet table, TetInfo[n_levels][6 N^3]
 };
 
 constexpr int REC_DOUBLES = 18;

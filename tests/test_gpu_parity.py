@@ -243,6 +243,35 @@ def test_patches_parity_and_refinement(psd, ctx, oracle):
     assert_mass(mass[l0].sum())
 
 
+def test_patches_with_shared_faces(psd, ctx, oracle):
+    """a7 with every face clipped once (PSD_OPT_FACE_SHARING; one per-tet table per level, the patch
+    masses in fixed point until the end, restriction after the conversion): against the oracle, and
+    the tet formulation, every chord axis, no restriction and accumulate = 1 (tet formulation again)
+    give the same."""
+    pos = crossing_field(16, 1.2, dtype="float32", stride=4, modes=40, kmax=4)
+    base_G, P, max_level, factor = 32, 16, 2, 1.5
+    ctx.psd_build_tets(to_dev(pos))
+    patches = ctx.psd_refine_patches(base_G, P, max_level, factor)
+    assert (patches[:, 0] == 1).any() and (patches[:, 0] == 2).any()
+    ora = oracle.deposit_patches(pos, 1.0, 1.0, base_G, P, patches)
+    mx = ora.max()
+    mass = ctx.psd_deposit_patches(patches, P, base_G).cpu().numpy()
+    assert ctx.psd_get_stats().shared_faces == 1
+    assert (np.abs(mass - ora) <= 1e-9 * mx + 1e-6 * np.abs(ora)).all()
+    for sharing, restrict in ((0, 1), (2, 1), (3, 0)):
+        ctx.psd_set_option(psd.OPT_FACE_SHARING, sharing)
+        ctx.psd_set_option(psd.OPT_PATCH_RESTRICT, restrict)
+        m2 = ctx.psd_deposit_patches(patches, P, base_G).cpu().numpy()
+        assert ctx.psd_get_stats().shared_faces == (1 if sharing else 0)
+        assert (np.abs(m2 - ora) <= 1e-9 * mx + 1e-6 * np.abs(ora)).all(), (sharing, restrict)
+    ctx.psd_set_option(psd.OPT_FACE_SHARING, 1)
+    ctx.psd_set_option(psd.OPT_PATCH_RESTRICT, 1)
+    acc = ctx.psd_deposit_patches(patches, P, base_G)
+    ctx.psd_deposit_patches(patches, P, base_G, acc, accumulate=True)
+    assert ctx.psd_get_stats().shared_faces == 0
+    assert (np.abs(acc.cpu().numpy() - 2.0 * ora) <= 2e-9 * mx + 2e-6 * np.abs(ora)).all()
+
+
 @pytest.mark.parametrize("N,B,dtype,stride", [(32, 8, "float32", 4), (40, 8, "float64", 3), (36, 8, "float32", 3),
                                               (32, 4, "float32", 4)])
 def test_subblock_census_bit_exact_and_drives_the_refinement(psd, ctx, oracle, N, B, dtype, stride):
@@ -672,6 +701,7 @@ def test_full_size_config_sampled_parity(psd, ctx, oracle, cfg_index, n_random, 
     check_windows(oracle, pos, grid, G, wins, edge, mx)
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    assert s.shared_faces == 1  # every face clipped once: the default path at full size
     ctx.psd_set_option(psd.OPT_WEIGHT_MODE, 1)
     ctx.psd_deposit_uniform(G, grid)
     assert float((grid - 1.0).abs().max()) < 1e-9
@@ -701,6 +731,7 @@ def test_cfg3_full_size_patches(psd, ctx, oracle):
     mass = ctx.psd_deposit_patches(patches, P, base_G)
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    assert s.shared_faces == 1  # every face clipped once: the default path at full size
     assert_mass(mass[torch.from_numpy(levels == 0).cuda()].sum())
     # sampled patches against the oracle: per level the hottest one (largest census count) and
     # four seeded ones
@@ -747,6 +778,7 @@ def test_cfg4_full_size_uniform(psd, ctx, oracle):
     ctx.psd_deposit_uniform(G, grid)
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 == 805306368 and s.n_degenerate == 0
+    assert s.shared_faces == 1  # every face clipped once: the default path at full size
     total = float(grid.sum())
     assert abs(total - 1.0) <= 1e-10, total
     assert float(grid.min()) > 0.0
@@ -795,6 +827,7 @@ def test_paper_weak_scaling_workload_at_its_quoted_size(psd, ctx, oracle):
     ctx.psd_deposit_uniform(G, grid)
     s = ctx.psd_get_stats()
     assert s.n_tets == 6 * cfg["N"] ** 3 and s.n_degenerate == 0
+    assert s.shared_faces == 1  # every face clipped once: the default path at full size
     assert_mass(grid.sum())
     assert float(grid.min()) > 0.0
     wins, _ = aimed_windows(oracle, pos, G, 12, 2, 1005)
