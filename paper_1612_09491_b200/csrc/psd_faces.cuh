@@ -263,15 +263,22 @@ __global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A
             unsigned long long word = (unsigned long long)ax | (unsigned long long)special << 2 | (unsigned long long)scell << 3 |
                                       (unsigned long long)(cloT | chiT << 3) << 12;
             unsigned int cnts = 0u;
+            // the four neighbours' table entries, all loads in flight before the first is used
+            TetInfo nbr[4];
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
                 const unsigned int nb = c_tet_nbr[t6][f];
-                // the neighbour behind face f: its table entry, its cell range in this tet's image
                 int ni = i + (int)(nb & 3u) - 1, nj = j + (int)((nb >> 2) & 3u) - 1, nk = k + (int)((nb >> 4) & 3u) - 1;
                 ni = ni < 0 ? ni + N : (ni >= N ? ni - N : ni);
                 nj = nj < 0 ? nj + N : (nj >= N ? nj - N : nj);
                 nk = nk < 0 ? nk + N : (nk >= N ? nk - N : nk);
-                const TetInfo en = tetinfo_load(info, (((int64_t)ni * N + nj) * N + nk) * 6 + (int)((nb >> 19) & 7u));
+                nbr[f] = tetinfo_load(info, (((int64_t)ni * N + nj) * N + nk) * 6 + (int)((nb >> 19) & 7u));
+            }
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {
+                const unsigned int nb = c_tet_nbr[t6][f];
+                // the neighbour behind face f: its cell range in this tet's image
+                const TetInfo en = nbr[f];
                 int nlo[3], nhi[3];
                 bool meets = true;
 #pragma unroll
