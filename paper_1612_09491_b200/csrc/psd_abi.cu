@@ -202,9 +202,23 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         k_items<<<(unsigned int)((n_tiles + 255) / 256), 256, 0, st>>>(
             ctx->tile_counts.as<unsigned int>(), n_tiles, ctx->chunk, ctx->tile_offsets.as<unsigned long long>(),
             ctx->item_offsets.as<unsigned long long>(), ctx->items.as<Item>());
-        k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
-                                             ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
-                                             nullptr, nullptr);
+        if (pair_share) {
+            // what a pair needs of its tet and the four neighbours (weight, cell range), per level; the
+            // scatter pass reads the cell ranges from it too
+            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)));
+            const double mass_per_tet = ctx->total_mass / (6.0 * (double)ncell);
+            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)g0 / space.L, top_level + 1,
+                                                                                mass_per_tet, ctx->weight_mode,
+                                                                                ctx->tet_info.as<TetInfo>());
+            ctx->launches += 1;
+            k_scatter_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
+                ctx->tet_info.as<TetInfo>(), 6 * ncell, space, ctx->tile_offsets.as<unsigned long long>(),
+                ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>());
+        } else {
+            k_census<true><<<cgrid, cb, 0, st>>>(ctx->part, space, nullptr, ctx->tile_offsets.as<unsigned long long>(),
+                                                 ctx->cursors.as<unsigned int>(), ctx->pair_ids.as<unsigned int>(),
+                                                 nullptr, nullptr);
+        }
         ctx->launches += 2;
         CK(cudaEventRecord(ctx->ev[3], st));
         DepositArgs A{};
@@ -236,14 +250,6 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             if (bound > 0.0 && std::isfinite(bound)) std::frexp(bound, &eb);  // bound < 2^eb
             A.acc_scale = std::ldexp(1.0, 62 - eb);
             A.acc_inv_scale = std::ldexp(1.0, -(62 - eb));
-            // what a pair needs of its tet and the four neighbours: determinant, cell range
-            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)));
-            for (int l = 0; l <= top_level; ++l) {
-                k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
-                    ctx->part, (double)(g0 << l) / space.L, A.mass_per_tet, ctx->weight_mode,
-                    ctx->tet_info.as<TetInfo>() + (size_t)l * (size_t)(6 * ncell));
-                ctx->launches += 1;
-            }
             A.tet_info = ctx->tet_info.p;
         }
         const size_t rec_bytes = pair_share ? sizeof(double) * REC2_DOUBLES : REC_BYTES;

@@ -159,30 +159,65 @@ __device__ __forceinline__ int tetinfo_lo(const TetInfo& e, int x) { return (int
 __device__ __forceinline__ int tetinfo_ext(const TetInfo& e, int x) { return (int)((e.box >> (36 + 9 * x)) & 511ull); }
 __device__ __forceinline__ bool tetinfo_one_cell(const TetInfo& e) { return ((e.box >> 36) & 0x7ffffffull) == 0ull; }
 __device__ __forceinline__ bool tetinfo_degenerate(const TetInfo& e) { return (e.box >> 63) != 0ull; }
-__global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scale, const double mass_per_tet,
-                                                  const int weight_mode, TetInfo* info) {
+// n_levels tables, one after the other (patch mode: level l has scale0 2^l cells per box length;
+// a power of two in the scale changes no rounding, so the determinant is 8^l times level 0's).
+__global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scale0, const int n_levels,
+                                                  const double mass_per_tet, const int weight_mode, TetInfo* info) {
     const int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
     const int64_t id = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (id >= ntet) return;
     double P[4][3];
     load_tet_vertices(p, id / 6, (int)(id % 6), P);
     Tet t;
-    finish_tet(P, scale, t);
-    const double det = tet_det(t.g);
-    TetInfo e;
-    e.val = weight_mode == 0 ? (det != 0.0 ? 6.0 * mass_per_tet / det : 0.0) : det;
-    e.box = (unsigned long long)(det == 0.0) << 63;
+    finish_tet(P, scale0, t);
+    const double det0 = tet_det(t.g);
+    for (int l = 0; l < n_levels; ++l) {
+        if (l) finish_tet(P, scale0 * (double)(1 << l), t);
+        const double det = det0 * (double)(1ll << (3 * l));
+        TetInfo e;
+        e.val = weight_mode == 0 ? (det != 0.0 ? 6.0 * mass_per_tet / det : 0.0) : det;
+        e.box = (unsigned long long)(det == 0.0) << 63;
 #pragma unroll
-    for (int x = 0; x < 3; ++x)
-        e.box |= (unsigned long long)((t.lo[x] + 1024) & 4095) << (12 * x) |
-                 (unsigned long long)min(t.hi[x] - t.lo[x], TETINFO_MAX_EXTENT) << (36 + 9 * x);
-    reinterpret_cast<double2*>(info)[id] = make_double2(e.val, __longlong_as_double((long long)e.box));
+        for (int x = 0; x < 3; ++x)
+            e.box |= (unsigned long long)((t.lo[x] + 1024) & 4095) << (12 * x) |
+                     (unsigned long long)min(t.hi[x] - t.lo[x], TETINFO_MAX_EXTENT) << (36 + 9 * x);
+        reinterpret_cast<double2*>(info)[(int64_t)l * ntet + id] = make_double2(e.val, __longlong_as_double((long long)e.box));
+    }
 }
 __device__ __forceinline__ TetInfo tetinfo_load(const TetInfo* info, int64_t id) {
     const double2 v = __ldg(reinterpret_cast<const double2*>(info) + id);
     TetInfo e;
     e.val = v.x; e.box = (unsigned long long)__double_as_longlong(v.y);
     return e;
+}
+
+// a3 with the table: the scatter pass of the counting sort from the tets' cell ranges in the
+// table instead of rebuilding every tet from its particles (k_census<true> does that): one thread
+// per tet, the same enumeration of tiles and the same size classes as the count pass.
+__global__ void __launch_bounds__(256) k_scatter_info(const TetInfo* info, const long long ntet, Space s,
+                                                      const unsigned long long* tile_offsets, unsigned int* cursors,
+                                                      unsigned int* pair_ids) {
+    const long long id = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (id >= ntet) return;
+    const int nlev = s.patch_mode ? s.n_levels : 1;
+    for (int level = 0; level < nlev; ++level) {
+        const TetInfo e = tetinfo_load(info + (long long)level * ntet, id);
+        int lo[3], hi[3];
+#pragma unroll
+        for (int x = 0; x < 3; ++x) { lo[x] = tetinfo_lo(e, x); hi[x] = lo[x] + tetinfo_ext(e, x); }
+        const int Gl = level_G(s, level);
+        for_each_block(lo, hi, Gl, TILE, Gl / TILE, [&](int tx, int ty, int tz, long long inside) {
+            const long long tid = tile_id_of(s, level, tx, ty, tz);
+            if (tid < 0) return;
+            const long long bin = tid * N_CLASSES + (inside > s.class_small_max ? 1 : 0);
+            const unsigned int peers = __match_any_sync(__activemask(), (unsigned int)bin);
+            const int leader = __ffs(peers) - 1;
+            unsigned int base = 0;
+            if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&cursors[bin], (unsigned int)__popc(peers));
+            base = __shfl_sync(peers, base, leader);
+            pair_ids[tile_offsets[bin] + base + __popc(peers & ((1u << (threadIdx.x & 31)) - 1u))] = (unsigned int)id;
+        });
+    }
 }
 
 // Record of a (tet, tile) pair, 23 doubles (184 bytes):
