@@ -86,8 +86,8 @@ def test_roofline_traffic_comes_from_the_committed_capture():
     assert isinstance(v, int) and v > 100e6
     assert bench.read_ncu_traffic("no_such_workload", "deposit") is None
     # the headline workload and the patch config have captures too (sums over the record slabs and
-    # over the kernels of the deposit phase: shared-face kernels on uniform grids, tet kernels on patches)
-    for w, main in (("cfg4_512_1024", "k_deposit_tiles2"), ("cfg3_256_patches", "k_deposit_tiles"),
+    # over the kernels of the deposit phase)
+    for w, main in (("cfg4_512_1024", "k_deposit_tiles2"), ("cfg3_256_patches", "k_deposit_tiles2"),
                     ("cfg2_256_512", "k_deposit_tiles2")):
         assert bench.read_ncu_traffic(w, "deposit") > bench.read_ncu_value(w, main) > 1e9
         assert bench.read_ncu_fp64_flops(w) > 1e11
