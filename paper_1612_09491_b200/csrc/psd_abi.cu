@@ -207,9 +207,12 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
             // scatter pass reads the cell ranges from it too
             CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)));
             const double mass_per_tet = ctx->total_mass / (6.0 * (double)ncell);
-            k_tet_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(ctx->part, (double)g0 / space.L, top_level + 1,
-                                                                                mass_per_tet, ctx->weight_mode,
-                                                                                ctx->tet_info.as<TetInfo>());
+            if (top_level > 0)
+                k_tet_info<true><<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
+                    ctx->part, (double)g0 / space.L, top_level + 1, mass_per_tet, ctx->weight_mode, ctx->tet_info.as<TetInfo>());
+            else
+                k_tet_info<false><<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
+                    ctx->part, (double)g0 / space.L, 1, mass_per_tet, ctx->weight_mode, ctx->tet_info.as<TetInfo>());
             ctx->launches += 1;
             k_scatter_info<<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
                 ctx->tet_info.as<TetInfo>(), 6 * ncell, space, ctx->tile_offsets.as<unsigned long long>(),

@@ -161,6 +161,7 @@ __device__ __forceinline__ bool tetinfo_one_cell(const TetInfo& e) { return ((e.
 __device__ __forceinline__ bool tetinfo_degenerate(const TetInfo& e) { return (e.box >> 63) != 0ull; }
 // n_levels tables, one after the other (patch mode: level l has scale0 2^l cells per box length;
 // a power of two in the scale changes no rounding, so the determinant is 8^l times level 0's).
+template <bool MULTI>  // false: one level (uniform grids), no loop: fewer registers
 __global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scale0, const int n_levels,
                                                   const double mass_per_tet, const int weight_mode, TetInfo* info) {
     const int64_t ntet = (int64_t)6 * p.N * p.N * p.N;
@@ -171,9 +172,10 @@ __global__ void __launch_bounds__(256) k_tet_info(Particles p, const double scal
     Tet t;
     finish_tet(P, scale0, t);
     const double det0 = tet_det(t.g);
-    for (int l = 0; l < n_levels; ++l) {
-        if (l) finish_tet(P, scale0 * (double)(1 << l), t);
-        const double det = det0 * (double)(1ll << (3 * l));
+    double s2 = 1.0, s8 = 1.0;  // 2^l, 8^l
+    for (int l = 0; l < (MULTI ? n_levels : 1); ++l, s2 *= 2.0, s8 *= 8.0) {
+        if (l) finish_tet(P, scale0 * s2, t);
+        const double det = l ? det0 * s8 : det0;
         TetInfo e;
         e.val = weight_mode == 0 ? (det != 0.0 ? 6.0 * mass_per_tet / det : 0.0) : det;
         e.box = (unsigned long long)(det == 0.0) << 63;
