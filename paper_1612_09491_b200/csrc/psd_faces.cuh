@@ -232,8 +232,11 @@ __global__ void __launch_bounds__(256) k_scatter_info(const TetInfo* info, const
 //   [22]     jobs per face, 8 bits each
 constexpr int REC2_DOUBLES = 23;
 constexpr int REC2_THREADS = 128;
+#ifndef REC2_MIN_CTAS
+#define REC2_MIN_CTAS 5
+#endif
 template <int ROWS>  // 0: rows in fp64, 1: in fp32
-__global__ void __launch_bounds__(REC2_THREADS, 5) k_pair_records2(DepositArgs A) {
+__global__ void __launch_bounds__(REC2_THREADS, REC2_MIN_CTAS) k_pair_records2(DepositArgs A) {
     constexpr int SS = 33;
     __shared__ unsigned long long stg[REC2_THREADS / 32][REC2_DOUBLES * SS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
