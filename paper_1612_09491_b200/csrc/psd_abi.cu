@@ -190,10 +190,13 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
     const int top_level = space.patch_mode ? space.n_levels - 1 : 0;
     const long long g0 = space.patch_mode ? space.base_G : space.G;
     const long long ext_top = (((long long)max_extent + 1) << top_level);
-    const bool pair_share = ctx->face_sharing && ctx->use_records && !ctx->accumulate_now && n_pairs > 0 &&
+    bool pair_share = ctx->face_sharing && ctx->use_records && !ctx->accumulate_now && n_pairs > 0 &&
                             2ll * (long long)max_extent + 2 + TILE < g0 && 2ll * ext_top + 2 + TILE < (g0 << top_level) &&
                             ext_top <= TETINFO_MAX_EXTENT && (g0 << top_level) <= 2048;
     const int face_axis = ctx->chord_axis >= 0 ? ctx->chord_axis : ctx->face_sharing - 1;
+    // (no room for the per-tet table: the tet formulation needs none)
+    if (pair_share && ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)) != cudaSuccess)
+        pair_share = false;
     ctx->last.shared_faces = pair_share ? 1 : 0;
     if (n_pairs > 0) {
         if (n_items > 0x7fffffffull) return fail(ctx, PSD_ERR_INVALID_ARG, "too many work items");
@@ -205,7 +208,6 @@ int run_binned(psd_ctx* ctx, Space space, long long n_tiles) {
         if (pair_share) {
             // what a pair needs of its tet and the four neighbours (weight, cell range), per level; the
             // scatter pass reads the cell ranges from it too
-            CK(ctx->tet_info.ensure(sizeof(TetInfo) * (size_t)(6 * ncell) * (size_t)(top_level + 1)));
             const double mass_per_tet = ctx->total_mass / (6.0 * (double)ncell);
             if (top_level > 0)
                 k_tet_info<true><<<(unsigned int)((6 * ncell + 255) / 256), 256, 0, st>>>(
